@@ -1,0 +1,77 @@
+"""The synthetic-input generator: structure, determinism, the statistics DESIGN.md quotes."""
+import numpy as np
+import torch
+
+from workloads import CONFIGS, DEFAULT_SEED, make_lists, make_probes, make_candidates, mini, make_codebooks, \
+    make_codes, encode_nearest, draw_vectors, stream_key
+
+
+def test_tiny_shapes_and_ranges(tiny_local):
+    w, c = tiny_local, tiny_local.cfg
+    assert w.queries.shape == (c.B, c.d) and w.queries.dtype == torch.float32
+    assert w.codebooks.shape == (c.M, 256, c.dsub)
+    assert w.codes.shape == (c.N, c.M) and w.codes.dtype == torch.uint8
+    assert w.cand_offsets.shape == (c.B + 1,) and w.cand_offsets.dtype == torch.int64
+    assert int(w.cand_offsets[0]) == 0 and int(w.cand_offsets[-1]) == w.cand_ids.numel()
+    ids = w.cand_ids.numpy()
+    assert ids.min() >= 0 and ids.max() < c.N
+    assert 780 <= w.stats["C_mean"] <= 820                       # "~800 IDs with duplicates"
+
+
+def test_lists_structure():
+    cfg = mini("i8_1b_m25", N=2_000_000, n_lists=4_000, B=8)
+    L = make_lists(cfg, DEFAULT_SEED)
+    off, ids = L.offsets.numpy(), L.ids.numpy()
+    assert off[-1] == ids.size and ids.min() >= 0 and ids.max() < cfg.N
+    for l in range(0, cfg.n_lists, 397):                         # IDs are unique inside a list
+        seg = ids[off[l]:off[l + 1]]
+        assert np.unique(seg).size == seg.size
+    copies = np.bincount(np.bincount(ids, minlength=cfg.N))
+    assert copies.size - 1 <= cfg.r_max                          # at most 8 lists
+    n_ref = copies[1:].sum()
+    assert n_ref == L.n_distinct
+    frac_rep = copies[2:].sum() / n_ref
+    assert abs(frac_rep - cfg.p_rep) < 0.01
+    assert abs(off[-1] / cfg.n_lists - cfg.mean_list) < 0.05 * cfg.mean_list
+    L2 = make_lists(cfg, DEFAULT_SEED, lists_per_chunk=1000)     # chunking does not change the result
+    assert torch.equal(L.ids, L2.ids) and torch.equal(L.offsets, L2.offsets)
+
+
+def test_candidates_are_the_probed_lists_concatenated():
+    cfg = mini("u8_10m_m32", N=500_000, n_lists=1_000, B=5)
+    L = make_lists(cfg, DEFAULT_SEED)
+    P = make_probes(cfg, DEFAULT_SEED)
+    assert P.shape == (cfg.B, cfg.nprobe)
+    for b in range(cfg.B):
+        assert P[b].unique().numel() == cfg.nprobe               # distinct lists
+    off, ids = make_candidates(cfg, L, P, max_chunk_ids=20_000)
+    off2, ids2 = make_candidates(cfg, L, P)
+    assert torch.equal(ids, ids2) and torch.equal(off, off2)
+    lo, li = L.offsets.numpy(), L.ids.numpy()
+    for b in range(cfg.B):
+        want = np.concatenate([li[lo[l]:lo[l + 1]] for l in P[b].tolist()])
+        assert np.array_equal(ids.numpy()[off[b]:off[b + 1]], want)
+    U = sum(np.unique(ids.numpy()[off[b]:off[b + 1]]).size for b in range(cfg.B))
+    assert 0.7 < U / int(off[-1]) < 0.9                          # ~0.82 distinct
+
+
+def test_histogram_codes_follow_the_encoded_distribution():
+    cfg = mini("u8_1b_m64", N=200_000, n_lists=400, B=2)
+    cb = make_codebooks(cfg, DEFAULT_SEED)
+    codes = make_codes(cfg, DEFAULT_SEED, cb, n_hist=1 << 14)
+    assert codes.shape == (cfg.N, cfg.M)
+    x = draw_vectors(cfg, stream_key(DEFAULT_SEED, cfg.name, "data"), 0, 1 << 14)
+    enc = encode_nearest(x, cb)
+    for m in (0, 31, 63):
+        h1 = np.bincount(codes[:, m].numpy(), minlength=256) / cfg.N
+        h2 = np.bincount(enc[:, m].numpy(), minlength=256) / enc.shape[0]
+        assert np.abs(h1 - h2).sum() < 0.15                      # same 256-way law (sampling noise)
+    assert np.bincount(codes[:, 0].numpy(), minlength=256).std() > 0   # not uniform
+
+
+def test_integer_configs_stay_integer():
+    for name in ("u8_10m_m32", "i8_1b_m25", "u8_1b_m64"):
+        cfg = CONFIGS[name]
+        cb = make_codebooks(cfg, DEFAULT_SEED)
+        assert torch.equal(cb, cb.round())
+        assert cfg.M * cfg.dsub * 255 ** 2 < 2 ** 24             # every ADC sum exact in fp32
