@@ -1,0 +1,200 @@
+/*
+ * fann.h -- C ABI of the B200-native GPU stage of FusionANNS (arxiv 2409.16576).
+ *
+ * The library runs, batched over queries on ONE GPU, the GPU side of the
+ * paper's CPU/GPU cooperative filtering (section 3 "Online
+ * Processing", L125-L133, Fig. 6 steps (1)(5)(6)(7)):
+ *
+ *   (1) per-query PQ distance lookup table          fann_build_lut
+ *   (5) dedup of the candidate vector-IDs   \
+ *   (6) gather PQ codes from HBM + Eq. 1     >      fann_dedup_scan_topk
+ *   (7) top-n candidates, ascending         /
+ *
+ * with the PQ codes pinned in HBM beforehand  fann_load_codes.
+ *
+ * Conventions
+ *   - Plain C.  No C++ or torch types cross this boundary.
+ *   - Every function that can fail returns a status (FANN_OK == 0, errors < 0)
+ *     and leaves a message for fann_last_error() (thread-local).  Nothing
+ *     throws, exits or allocates inside fann_build_lut / fann_dedup_scan_topk.
+ *   - "device pointer" = CUDA device memory of the index's device; "host
+ *     pointer" = ordinary (ideally pinned) host memory.  Each argument says which.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *     stream).  Calls only ENQUEUE work and return without synchronising,
+ *     unless stated otherwise.
+ *   - Ownership: the index owns only its private copy of the PQ codes.
+ *     Queries, codebooks, tables, candidate lists, outputs and workspace are
+ *     caller-owned and must stay valid until the enqueued work has finished.
+ *   - Distance is squared L2 (reading R1).  IDs are uint32.
+ *     FANN_ID_NONE in a candidate list is skipped; an ID >= N is dropped.
+ *   - There is no CPU fallback.  If no usable CUDA device exists the calls
+ *     fail with FANN_ECUDA.
+ */
+#ifndef FANN_H
+#define FANN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fann_index fann_index;          /* opaque, library-owned */
+
+enum {
+    FANN_OK           =  0,
+    FANN_EINVAL       = -1,   /* bad argument (NULL, zero size, mismatched M, ...)        */
+    FANN_ECUDA        = -2,   /* CUDA runtime error; message has the CUDA error string   */
+    FANN_ENOMEM       = -3,   /* device allocation failed                                 */
+    FANN_EUNSUPPORTED = -4,   /* M > FANN_MAX_M, k > FANN_MAX_K, dsub == 0, ...           */
+    FANN_EWORKSPACE   = -5,   /* workspace NULL, misaligned or smaller than required      */
+    FANN_EOVERFLOW    = -6    /* reported by fann_workspace_status: a dedup table filled  */
+};
+
+#define FANN_ID_NONE 0xFFFFFFFFu               /* padding in candidate lists and in outputs */
+#define FANN_MAX_M   64u                       /* PQ bytes per vector (lookup table <= 64 KB) */
+#define FANN_MAX_K   1024u                     /* candidates returned per query             */
+
+/* Create an index on CUDA device `device`.  *out receives the handle. */
+int  fann_create(fann_index **out, int device);
+/* Free the index and its copy of the codes.  Synchronises the device. NULL is a no-op. */
+void fann_destroy(fann_index *ix);
+/* Message of the last failing call made by this host thread.  Never NULL. */
+const char *fann_last_error(void);
+/* "fann <version> sm_100a". */
+const char *fann_version(void);
+
+/*
+ * PAPER.md:L152 "we pin all compressed vectors in the HBM".
+ * Copy rows [first, first+n) of the N_total x M uint8 PQ code array (row-major,
+ * `codes` points at row `first`) into library-owned HBM.  The library stores
+ * rows padded to a multiple of 16 bytes (M=25 -> 32) so that every row is read
+ * with aligned 16-byte loads; padding bytes are zero and never contribute.
+ * The first call fixes N_total and M and allocates; later calls must repeat
+ * them and may load other row ranges (so 25-64 GB can be streamed in chunks).
+ * codes: host pointer if src_is_device == 0, else device pointer.
+ * For a host source the call synchronises `stream` before returning.
+ * Errors: EINVAL (NULL, range outside N_total, M or N_total changed, M == 0),
+ * EUNSUPPORTED (M > FANN_MAX_M, N_total >= 2^32), ENOMEM, ECUDA.
+ */
+int fann_load_codes(fann_index *ix, const uint8_t *codes, uint64_t first, uint64_t n,
+                    uint64_t N_total, uint32_t M, int src_is_device, void *stream);
+
+/*
+ * Step (1): the distance lookup table
+ *     lut[b][m][j] = sum_{t<dsub} (queries[b][m*dsub+t] - codebooks[m][j][t])^2
+ * in fp32, direct form (no norm expansion).  M is the index's M (codes must be
+ * loaded first); d = M*dsub.
+ * queries   device pointer, [B][d] fp32 row-major
+ * codebooks device pointer, [M][256][dsub] fp32
+ * lut       device pointer, [B][M][256] fp32, written
+ * Errors: EINVAL (NULL, B == 0, codes not loaded), EUNSUPPORTED (dsub == 0 or > 64).
+ */
+int fann_build_lut(fann_index *ix, const float *queries, uint32_t B,
+                   const float *codebooks, uint32_t dsub, float *lut, void *stream);
+
+/*
+ * Bytes of device workspace fann_dedup_scan_topk / fann_dedup_only need for a
+ * batch of B queries holding total_cands candidate IDs in all.  The workspace
+ * is the paper's per-query working memory turned inside out:
+ * the caller allocates it once and reuses it across batches.  Returns 0 on a
+ * bad argument (see fann_last_error).
+ */
+size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t total_cands, uint32_t k);
+
+/*
+ * Steps (5)(6)(7), for a batch.  For every query b:
+ *   (5) the set of distinct valid IDs among cand_ids[cand_offsets[b] .. cand_offsets[b+1])
+ *   (6) Eq. 1: dist(v) = sum_m lut[b][m][codes[v][m]], fp32
+ *       (summation order unspecified; exact whenever all partial sums are
+ *       integers below 2^24)
+ *   (7) the min(k, U_b) smallest (dist, id) pairs, ordered by dist ascending,
+ *       then id ascending; the remaining slots hold (+inf, FANN_ID_NONE).
+ * lut          device, [B][M][256] fp32 as written by fann_build_lut
+ * cand_offsets device, [B+1] int64, non-decreasing, cand_offsets[0] == 0
+ * cand_ids     device, [total_cands] uint32
+ * total_cands  host value == cand_offsets[B] (lets the call size its work
+ *              without reading device memory)
+ * out_ids      device, [B][k] uint32        out_dists  device, [B][k] fp32
+ * out_counts   device, [B] uint32 = min(k, U_b); may be NULL
+ * out_uniq     device, [B] uint32 = U_b (distinct valid IDs scored); may be NULL
+ * workspace    device, >= fann_workspace_bytes(ix, B, total_cands, k), 256-byte aligned
+ * Synchronous errors: EINVAL, EUNSUPPORTED (k == 0 or k > FANN_MAX_K),
+ * EWORKSPACE.  Asynchronous conditions are left in the workspace and read
+ * with fann_workspace_status.
+ */
+int fann_dedup_scan_topk(fann_index *ix, const float *lut, uint32_t B,
+                         const int64_t *cand_offsets, const uint32_t *cand_ids,
+                         uint64_t total_cands, uint32_t k,
+                         uint32_t *out_ids, float *out_dists,
+                         uint32_t *out_counts, uint32_t *out_uniq,
+                         void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Step (5) alone, through the same kernel and hash tables as the call above
+ * (test hook for the bit-exact dedup check): the distinct valid IDs of query b,
+ * in any order, are written to uniq_ids[cand_offsets[b] .. +uniq_counts[b]).
+ * uniq_ids device, [total_cands] uint32; uniq_counts device, [B] uint32.
+ */
+int fann_dedup_only(fann_index *ix, uint32_t B, const int64_t *cand_offsets,
+                    const uint32_t *cand_ids, uint64_t total_cands,
+                    uint32_t *uniq_ids, uint32_t *uniq_counts,
+                    void *workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Synchronises `stream` and returns the status the last fann_dedup_scan_topk /
+ * fann_dedup_only left in `workspace`: FANN_OK, or FANN_EOVERFLOW if some
+ * query's dedup table filled up (only possible for candidate IDs chosen to
+ * collide under the library's hash; that query's outputs are then invalid).
+ */
+int fann_workspace_status(fann_index *ix, const void *workspace, void *stream);
+
+/*
+ * The whole stage from HOST buffers, for callers that hold the batch in host
+ * memory (the paper's step (4): the CPU sends the vector-IDs):
+ * copies queries / candidate lists host->device into `device_scratch`, runs
+ * fann_build_lut + fann_dedup_scan_topk, copies ids/dists/counts back and
+ * synchronises `stream` before returning.  Codebooks stay on the device.
+ * queries_h, cand_offsets_h, cand_ids_h, out_*_h: host pointers (pinned memory
+ * gives asynchronous copies); layouts as above.  out_counts_h may be NULL.
+ * device_scratch: device, >= fann_search_host_scratch_bytes(...), 256-byte aligned.
+ */
+size_t fann_search_host_scratch_bytes(const fann_index *ix, uint32_t B, uint32_t dsub,
+                                      uint64_t total_cands, uint32_t k);
+int fann_search_host(fann_index *ix, const float *queries_h, uint32_t B,
+                     const float *codebooks_d, uint32_t dsub,
+                     const int64_t *cand_offsets_h, const uint32_t *cand_ids_h,
+                     uint32_t k, uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h,
+                     void *device_scratch, size_t scratch_bytes, void *stream);
+
+/* Geometry and counters, for benchmarks and tests. */
+typedef struct fann_info {
+    uint64_t N;               /* rows loaded (N_total), 0 before fann_load_codes       */
+    uint32_t M;               /* PQ bytes per vector                                    */
+    uint32_t row_bytes;       /* stored row stride (M rounded up to 16)                 */
+    uint32_t num_sms;         /* multiprocessors of the device                          */
+    uint32_t scan_threads;    /* threads per CTA of the scan kernel                     */
+    uint32_t scan_ctas;       /* persistent CTAs of the last scan launch                */
+    uint32_t scan_smem_bytes; /* dynamic shared memory per CTA of the last scan launch  */
+    uint32_t table_slots;     /* dedup hash-table slots per CTA of the last scan launch */
+    uint64_t kernel_launches; /* kernels this index has launched so far                 */
+} fann_info;
+int fann_get_info(const fann_index *ix, fann_info *out);
+
+/*
+ * Per-kernel device timing for benchmarks.  With enable != 0 every later
+ * fann_build_lut / fann_dedup_scan_topk records CUDA events on the launching
+ * stream around its kernels.  fann_last_timing synchronises on the last of
+ * those events and returns the durations in milliseconds of the most recent
+ * lookup-table kernel, plan kernel, scan kernel (dedup + gather + ADC + local
+ * top-k) and merge kernel; a value is -1 if that kernel has not run since
+ * timing was enabled.  Any pointer may be NULL.
+ */
+int fann_set_timing(fann_index *ix, int enable);
+int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *scan_ms, float *merge_ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FANN_H */

@@ -1,0 +1,280 @@
+"""CUDA path vs CPU oracle, through the C ABI (python binding = marshalling only).
+
+Integer-valued workloads: byte equality.  Real-valued workloads: the tolerance rules of
+DESIGN.md "Parity rules" (1e-5 relative, ties within the band may permute)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from parity import NONE, check_band, check_exact, check_lut
+from workloads import CONFIGS, make_workload, mini
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def fann():
+    import paper_2409_16576_b200 as f
+    from paper_2409_16576_b200.build import build
+    build()
+    f.load_library()
+    return f
+
+
+def np_u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def gpu_search(fann, w, k=None, cand=None, check=True):
+    """Run the whole path on the GPU.  cand = (offsets int64 np, ids uint32 np) overrides w's lists."""
+    k = k or w.cfg.k
+    ix = fann.FannIndex(0)
+    ix.load_codes(w.codes.to(DEV))
+    q, cb = w.queries.to(DEV), w.codebooks.to(DEV)
+    if cand is None:
+        off, ids = w.cand_offsets.to(DEV), w.cand_ids.to(DEV)
+    else:
+        off = torch.from_numpy(np.ascontiguousarray(cand[0], dtype=np.int64)).to(DEV)
+        ids = torch.from_numpy(np.ascontiguousarray(cand[1], dtype=np.uint32).view(np.int32)).to(DEV)
+        q = q[: off.numel() - 1].contiguous()
+    lut = ix.build_lut(q, cb)
+    o = ix.dedup_scan_topk(lut, off, ids, k, check=check)
+    torch.cuda.synchronize()
+    res = (np_u32(o[0]), o[1].cpu().numpy(), np_u32(o[2]), np_u32(o[3]))
+    return ix, lut, res
+
+
+def orc_search(w, k=None, cand=None):
+    k = k or w.cfg.k
+    q = w.queries.numpy()
+    if cand is None:
+        off, ids = w.cand_offsets.numpy(), w.cand_ids.numpy().view(np.uint32)
+    else:
+        off, ids = cand
+        q = q[: len(off) - 1]
+    return oracle.search(q, w.codebooks.numpy(), w.codes.numpy(), off, ids, k)
+
+
+def band_all(w, res, k=None, cand=None):
+    k = k or w.cfg.k
+    if cand is None:
+        off, ids = w.cand_offsets.numpy(), w.cand_ids.numpy().view(np.uint32)
+    else:
+        off, ids = cand
+    needed = 0
+    for b in range(len(off) - 1):
+        ai, ad = oracle.query_all(w.queries.numpy()[b], w.codebooks.numpy(), w.codes.numpy(), ids[off[b]:off[b + 1]])
+        assert res[3][b] == ai.size, f"query {b}: uniq {res[3][b]} != {ai.size}"
+        needed += check_band(res[0][b], res[1][b], res[2][b], ai, ad, k)
+    return needed
+
+
+# ------------------------------------------------------------------ workloads
+
+@pytest.fixture(scope="module")
+def w_int():
+    """configs[1] structure (uint8 data, M=32, k=100) at a size the oracle finishes in seconds;
+    ~32k candidates per query -> several table partitions, ragged tails."""
+    return make_workload(mini("u8_10m_m32", N=400_000, n_lists=800, B=24, codes_mode="histogram"))
+
+
+@pytest.fixture(scope="module")
+def w_i8():
+    """configs[3] structure (int8, M=25 -> rows padded to 32 bytes, power-law lists)."""
+    return make_workload(mini("i8_1b_m25", N=300_000, n_lists=600, B=16))
+
+
+@pytest.fixture(scope="module")
+def w_k1000():
+    """configs[4] structure (M=64, nprobe=256, k=1000): ~128k candidates per query."""
+    return make_workload(mini("u8_1b_m64", N=600_000, n_lists=1_200, B=6))
+
+
+@pytest.fixture(scope="module")
+def w_f32():
+    """configs[2] structure (fp32 Gaussian normalised, M=48): tolerance regime."""
+    return make_workload(mini("f32_100m_m48", N=300_000, n_lists=600, B=8))
+
+
+# ------------------------------------------------------------------ (1) lookup table
+
+@pytest.mark.parametrize("name", ["tiny", "tiny_local"])
+def test_lut_tiny(fann, name, request):
+    w = request.getfixturevalue(name)
+    ix = fann.FannIndex(0)
+    ix.load_codes(w.codes.to(DEV))
+    lut = ix.build_lut(w.queries.to(DEV), w.codebooks.to(DEV)).cpu().numpy()
+    check_lut(lut, oracle.build_lut(w.queries.numpy(), w.codebooks.numpy()))
+
+
+def test_lut_integer_exact_and_fp32(fann, w_int, w_f32, w_i8):
+    for w in (w_int, w_i8, w_f32):
+        ix = fann.FannIndex(0)
+        ix.load_codes(w.codes[:1000].contiguous().to(DEV))
+        lut = ix.build_lut(w.queries.to(DEV), w.codebooks.to(DEV)).cpu().numpy()
+        lut64 = oracle.build_lut(w.queries.numpy(), w.codebooks.numpy())
+        check_lut(lut, lut64)
+        if w.cfg.integer_exact:
+            assert np.array_equal(lut.astype(np.float64), lut64)
+
+
+def test_lut_query_on_centroid_is_exact_zero(fann, tiny):
+    w = tiny
+    q = w.queries.clone()
+    q[0] = w.codebooks[:, 17, :].reshape(-1)
+    ix = fann.FannIndex(0)
+    ix.load_codes(w.codes[:100].contiguous().to(DEV))
+    lut = ix.build_lut(q.to(DEV), w.codebooks.to(DEV)).cpu().numpy()
+    assert np.all(lut[0, :, 17] == 0.0) and np.all(lut >= 0)
+
+
+# ------------------------------------------------------------------ (5) dedup
+
+def _dedup_check(fann, w, off, ids):
+    ix = fann.FannIndex(0)
+    ix.load_codes(w.codes.to(DEV))
+    o = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int64)).to(DEV)
+    i = torch.from_numpy(np.ascontiguousarray(ids, dtype=np.uint32).view(np.int32)).to(DEV)
+    uids, ucnt = ix.dedup_only(o, i)
+    torch.cuda.synchronize()
+    uids, ucnt = np_u32(uids), np_u32(ucnt)
+    for b in range(len(off) - 1):
+        want = oracle.dedup(ids[off[b]:off[b + 1]], w.cfg.N)
+        got = uids[off[b]:off[b] + ucnt[b]]
+        assert ucnt[b] == want.size, f"query {b}: {ucnt[b]} != {want.size}"
+        assert np.array_equal(np.sort(got), want), f"query {b}: distinct sets differ"
+
+
+def test_dedup_sets_bit_exact(fann, tiny_local, w_int, w_k1000):
+    for w in (tiny_local, w_int, w_k1000):
+        _dedup_check(fann, w, w.cand_offsets.numpy(), w.cand_ids.numpy().view(np.uint32))
+
+
+def test_dedup_adversarial(fann, tiny_local):
+    w = tiny_local
+    N = w.cfg.N
+    rng = np.random.default_rng(5)
+    lists = [
+        np.full(5000, 4242, dtype=np.uint32),                                   # all duplicates
+        np.arange(3000, dtype=np.uint32),                                       # no duplicate
+        np.array([], dtype=np.uint32),                                          # empty
+        np.full(100, NONE, dtype=np.uint32),                                    # only padding
+        np.array([N, N + 1, 2 ** 31, NONE - 1, 5], dtype=np.uint32),            # out of range except one
+        rng.integers(0, 50, size=40_000).astype(np.uint32),                     # 50 ids, long list
+        np.concatenate([rng.permutation(N)[:60_000].astype(np.uint32)] * 2),    # 120k, each twice
+    ]
+    off = np.zeros(len(lists) + 1, dtype=np.int64)
+    off[1:] = np.cumsum([len(x) for x in lists])
+    _dedup_check(fann, w, off, np.concatenate(lists))
+
+
+# ------------------------------------------------------------------ whole path
+
+def test_tiny_configs_tolerance_regime(fann, tiny, tiny_local):
+    for w in (tiny, tiny_local):
+        _, _, res = gpu_search(fann, w)
+        band_all(w, res)
+
+
+def test_integer_exact_configs_bytes(fann, w_int, w_i8):
+    for w in (w_int, w_i8):
+        ix, _, res = gpu_search(fann, w)
+        check_exact(res, orc_search(w))
+        assert ix.info()["kernel_launches"] >= 4
+
+
+def test_k1000_partitions_bytes(fann, w_k1000):
+    w = w_k1000
+    _, _, res = gpu_search(fann, w)
+    ref = orc_search(w)
+    check_exact(res, ref)
+    assert ref["uniq"].min() > 1000                      # k < U: selection really happens
+    # integer data: exact ties inside the top-1000 exist and are ordered by id
+    ties = sum(int(np.sum(np.diff(ref["dists"][b]) == 0)) for b in range(w.cfg.B))
+    assert ties > 0
+
+
+def test_fp32_config_band(fann, w_f32):
+    _, _, res = gpu_search(fann, w_f32)
+    band_all(w_f32, res)
+
+
+def test_edge_cases(fann, w_int):
+    w = w_int
+    N = w.cfg.N
+    rng = np.random.default_rng(9)
+    base = w.cand_ids.numpy().view(np.uint32)[: int(w.cand_offsets[1])]
+    lists = [
+        np.array([], dtype=np.uint32),                                          # empty list -> count 0
+        base[:37],                                                              # fewer than k distinct
+        np.full(2000, base[3], dtype=np.uint32),                                # one distinct id
+        np.concatenate([[NONE] * 5, base[:500], [N, N + 7], [NONE] * 3]).astype(np.uint32),
+        base,                                                                   # a normal list
+        np.concatenate([base, base]),                                           # appended to itself
+        rng.permutation(base),                                                  # permuted
+        rng.permutation(N)[:150_000].astype(np.uint32),                         # max-skew: 150k distinct
+    ]
+    off = np.zeros(len(lists) + 1, dtype=np.int64)
+    off[1:] = np.cumsum([len(x) for x in lists])
+    cand = (off, np.concatenate(lists))
+    for k in (100, 1, 1024, 7):
+        _, _, res = gpu_search(fann, w, k=k, cand=cand)
+        ref = orc_search(w, k=k, cand=cand)
+        check_exact(res, ref)
+        assert res[2][0] == 0 and np.all(res[0][0] == NONE) and np.all(np.isposinf(res[1][0]))
+        assert res[2][2] == 1
+        for a, b in ((4, 5), (4, 6)):                                           # metamorphic
+            assert np.array_equal(res[0][a], res[0][b]) and np.array_equal(res[1][a], res[1][b])
+
+
+def test_argument_errors(fann, tiny):
+    w = tiny
+    ix = fann.FannIndex(0)
+    with pytest.raises(fann.FannError):                                         # no codes yet
+        fann.fann_workspace_bytes(ix.handle, 4, 100, 10)
+    ix.load_codes(w.codes[:1000].contiguous().to(DEV))
+    lut = ix.build_lut(w.queries.to(DEV), w.codebooks.to(DEV))
+    off, ids = w.cand_offsets.to(DEV), w.cand_ids.to(DEV)
+    with pytest.raises(fann.FannError) as e:
+        ix.dedup_scan_topk(lut, off, ids, k=fann.FANN_MAX_K + 1)
+    assert e.value.code in (-1, -4)
+    B = w.cfg.B
+    out = [torch.empty((B, 10), dtype=torch.int32, device=DEV), torch.empty((B, 10), device=DEV)]
+    small = torch.empty(256, dtype=torch.uint8, device=DEV)
+    with pytest.raises(fann.FannError) as e:
+        fann.fann_dedup_scan_topk(ix.handle, lut, B, off, ids, ids.numel(), 10, out[0], out[1], None, None,
+                                  small, small.numel())
+    assert e.value.code == -5
+    with pytest.raises(fann.FannError):
+        ix.load_codes(w.codes[:10, :8].contiguous().to(DEV))                    # M changed
+
+
+def test_host_entry_matches_device_entry(fann, w_i8):
+    w = w_i8
+    ix, _, res = gpu_search(fann, w)
+    B, k, total = w.cfg.B, w.cfg.k, w.cand_ids.numel()
+    need = fann.fann_search_host_scratch_bytes(ix.handle, B, w.cfg.dsub, total, k)
+    scratch = torch.empty(need, dtype=torch.uint8, device=DEV)
+    q_h, off_h, ids_h = w.queries.pin_memory(), w.cand_offsets.pin_memory(), w.cand_ids.pin_memory()
+    oi = torch.empty((B, k), dtype=torch.int32).pin_memory()
+    od = torch.empty((B, k), dtype=torch.float32).pin_memory()
+    oc = torch.empty(B, dtype=torch.int32).pin_memory()
+    fann.fann_search_host(ix.handle, q_h, B, w.codebooks.to(DEV), w.cfg.dsub, off_h, ids_h, k, oi, od, oc,
+                          scratch, need, torch.cuda.current_stream().cuda_stream)
+    assert np.array_equal(oi.numpy().view(np.uint32), res[0])
+    assert np.array_equal(od.numpy(), res[1]) and np.array_equal(oc.numpy().view(np.uint32), res[2])
+
+
+def test_load_codes_from_host_and_in_chunks(fann, w_i8):
+    w = w_i8
+    ix = fann.FannIndex(0)
+    N = w.cfg.N
+    half = N // 2
+    ix.load_codes(w.codes[:half].contiguous(), first=0, N_total=N)             # host source, padded rows
+    ix.load_codes(w.codes[half:].contiguous().to(DEV), first=half, N_total=N)  # device source
+    lut = ix.build_lut(w.queries.to(DEV), w.codebooks.to(DEV))
+    o = ix.dedup_scan_topk(lut, w.cand_offsets.to(DEV), w.cand_ids.to(DEV), w.cfg.k, check=True)
+    torch.cuda.synchronize()
+    check_exact((np_u32(o[0]), o[1].cpu().numpy(), np_u32(o[2]), np_u32(o[3])), orc_search(w))
