@@ -27,12 +27,12 @@ def np_u32(t):
     return t.cpu().numpy().view(np.uint32)
 
 
-def gpu_search(fann, w, k=None, cand=None, check=True):
+def gpu_search(fann, w, k=None, cand=None, check=True, queries=None):
     """Run the whole path on the GPU.  cand = (offsets int64 np, ids uint32 np) overrides w's lists."""
     k = k or w.cfg.k
     ix = fann.FannIndex(0)
     ix.load_codes(w.codes.to(DEV))
-    q, cb = w.queries.to(DEV), w.codebooks.to(DEV)
+    q, cb = (w.queries if queries is None else queries).to(DEV), w.codebooks.to(DEV)
     if cand is None:
         off, ids = w.cand_offsets.to(DEV), w.cand_ids.to(DEV)
     else:
@@ -46,9 +46,9 @@ def gpu_search(fann, w, k=None, cand=None, check=True):
     return ix, lut, res
 
 
-def orc_search(w, k=None, cand=None):
+def orc_search(w, k=None, cand=None, queries=None):
     k = k or w.cfg.k
-    q = w.queries.numpy()
+    q = (w.queries if queries is None else queries).numpy()
     if cand is None:
         off, ids = w.cand_offsets.numpy(), w.cand_ids.numpy().view(np.uint32)
     else:
@@ -219,9 +219,12 @@ def test_edge_cases(fann, w_int):
     off = np.zeros(len(lists) + 1, dtype=np.int64)
     off[1:] = np.cumsum([len(x) for x in lists])
     cand = (off, np.concatenate(lists))
+    q = w.queries.clone()
+    q[5] = q[4]                                                                 # same query for the
+    q[6] = q[4]                                                                 # metamorphic triple
     for k in (100, 1, 1024, 7):
-        _, _, res = gpu_search(fann, w, k=k, cand=cand)
-        ref = orc_search(w, k=k, cand=cand)
+        _, _, res = gpu_search(fann, w, k=k, cand=cand, queries=q)
+        ref = orc_search(w, k=k, cand=cand, queries=q)
         check_exact(res, ref)
         assert res[2][0] == 0 and np.all(res[0][0] == NONE) and np.all(np.isposinf(res[1][0]))
         assert res[2][2] == 1
