@@ -184,7 +184,7 @@ def main():
     launches0 = ix.info()["kernel_launches"]
     sampler = ClockSampler(local_rank) if rank == 0 else None
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern = {"lut_ms": [], "plan_ms": [], "scan_ms": [], "merge_ms": []}
+    kern = {"lut_ms": [], "plan_ms": [], "dedup_ms": [], "scan_ms": []}
     barrier()
     t0 = time.time()
     for i in range(args.steps):
@@ -300,7 +300,7 @@ def main():
         "input_ids_per_s": C_all / (ms_per_step * 1e-3),
         "hbm_frac_nominal_8TBs": round(achieved / 8000.0, 4),
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
-        "clocks": clocks, "scan_geometry": {kk: v for kk, v in ix.info().items() if kk.startswith(("scan_", "table_", "row_"))},
+        "clocks": clocks, "geometry": {kk: v for kk, v in ix.info().items() if kk.startswith(("scan_", "dedup_", "table_", "row_", "chunks"))},
     }
     print(json.dumps(line))
     if world > 1:

@@ -69,8 +69,9 @@ const char *fann_version(void);
  * PAPER.md:L152 "we pin all compressed vectors in the HBM".
  * Copy rows [first, first+n) of the N_total x M uint8 PQ code array (row-major,
  * `codes` points at row `first`) into library-owned HBM.  The library stores
- * rows padded to a multiple of 16 bytes (M=25 -> 32) so that every row is read
- * with aligned 16-byte loads; padding bytes are zero and never contribute.
+ * rows padded to 16, 32 or 64 bytes (M=25 -> 32, M=48 -> 64) so that a row never
+ * straddles a 64-byte DRAM access and is read with aligned 16-byte loads by 1, 2
+ * or 4 adjacent lanes; padding bytes are zero and never contribute.
  * The first call fixes N_total and M and allocates; later calls must repeat
  * them and may load other row ranges (so 25-64 GB can be streamed in chunks).
  * codes: host pointer if src_is_device == 0, else device pointer.
@@ -170,29 +171,47 @@ int fann_search_host(fann_index *ix, const float *queries_h, uint32_t B,
 
 /* Geometry and counters, for benchmarks and tests. */
 typedef struct fann_info {
-    uint64_t N;               /* rows loaded (N_total), 0 before fann_load_codes       */
-    uint32_t M;               /* PQ bytes per vector                                    */
-    uint32_t row_bytes;       /* stored row stride (M rounded up to 16)                 */
-    uint32_t num_sms;         /* multiprocessors of the device                          */
-    uint32_t scan_threads;    /* threads per CTA of the scan kernel                     */
-    uint32_t scan_ctas;       /* persistent CTAs of the last scan launch                */
-    uint32_t scan_smem_bytes; /* dynamic shared memory per CTA of the last scan launch  */
-    uint32_t table_slots;     /* dedup hash-table slots per CTA of the last scan launch */
-    uint64_t kernel_launches; /* kernels this index has launched so far                 */
+    uint64_t N;                /* rows loaded (N_total), 0 before fann_load_codes            */
+    uint32_t M;                /* PQ bytes per vector                                         */
+    uint32_t row_bytes;        /* stored row stride: 16, 32 or 64                             */
+    uint32_t num_sms;          /* multiprocessors of the device                               */
+    uint32_t dedup_threads;    /* threads per CTA of the dedup kernel                         */
+    uint32_t dedup_ctas;       /* persistent CTAs of the last dedup launch                    */
+    uint32_t dedup_smem_bytes; /* dynamic shared memory per dedup CTA                         */
+    uint32_t table_slots;      /* dedup hash-table slots one CTA can hold                     */
+    uint32_t scan_threads;     /* threads per CTA of the scan kernel                          */
+    uint32_t scan_ctas;        /* persistent CTAs of the last scan launch                     */
+    uint32_t scan_smem_bytes;  /* dynamic shared memory per scan CTA                          */
+    uint32_t scan_buffer_keys; /* top-k candidate buffer of a scan CTA, in (dist, id) keys    */
+    uint32_t chunks;           /* batch chunks of the last call (dedup i+1 beside scan i)     */
+    uint32_t reserved;
+    uint64_t kernel_launches;  /* kernels this index has launched so far                      */
 } fann_info;
 int fann_get_info(const fann_index *ix, fann_info *out);
 
 /*
  * Per-kernel device timing for benchmarks.  With enable != 0 every later
- * fann_build_lut / fann_dedup_scan_topk records CUDA events on the launching
- * stream around its kernels.  fann_last_timing synchronises on the last of
- * those events and returns the durations in milliseconds of the most recent
- * lookup-table kernel, plan kernel, scan kernel (dedup + gather + ADC + local
- * top-k) and merge kernel; a value is -1 if that kernel has not run since
- * timing was enabled.  Any pointer may be NULL.
+ * fann_build_lut / fann_dedup_scan_topk records CUDA events around its kernels on
+ * the stream each kernel is launched on.  fann_last_timing synchronises on the last
+ * of those events and returns, in milliseconds, the duration of the most recent
+ * lookup-table kernel and plan kernel and the summed durations of the dedup
+ * launches and of the scan launches (gather + ADC + top-k) of the most recent call;
+ * a value is -1 if that kernel has not run since timing was enabled.  When the call
+ * ran in several chunks, dedup and scan launches overlap in time, so the two sums
+ * can exceed the call's wall time.  Any pointer may be NULL.
  */
 int fann_set_timing(fann_index *ix, int enable);
-int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *scan_ms, float *merge_ms);
+int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup_ms, float *scan_ms);
+
+/*
+ * Measurement only: read the stored code rows of
+ * ids[0 .. n) with the scan kernel's access pattern (the same lanes per row, loads
+ * in flight and threads per CTA) and do nothing else.  Timed by the caller, it
+ * gives the rate at which this GPU can gather those rows at all -- the practical
+ * ceiling of step (6).  IDs >= N read row 0.
+ * ids  device, [n] uint32      sink  device, 4 bytes (never written in practice)
+ */
+int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink, void *stream);
 
 #ifdef __cplusplus
 }

@@ -32,8 +32,10 @@ class FannError(RuntimeError):
 
 class _Info(C.Structure):
     _fields_ = [("N", C.c_uint64), ("M", C.c_uint32), ("row_bytes", C.c_uint32), ("num_sms", C.c_uint32),
-                ("scan_threads", C.c_uint32), ("scan_ctas", C.c_uint32), ("scan_smem_bytes", C.c_uint32),
-                ("table_slots", C.c_uint32), ("kernel_launches", C.c_uint64)]
+                ("dedup_threads", C.c_uint32), ("dedup_ctas", C.c_uint32), ("dedup_smem_bytes", C.c_uint32),
+                ("table_slots", C.c_uint32), ("scan_threads", C.c_uint32), ("scan_ctas", C.c_uint32),
+                ("scan_smem_bytes", C.c_uint32), ("scan_buffer_keys", C.c_uint32), ("chunks", C.c_uint32),
+                ("reserved", C.c_uint32), ("kernel_launches", C.c_uint64)]
 
 
 def library_path() -> str:
@@ -67,6 +69,7 @@ def load_library():
         "fann_get_info": (i, [p, C.POINTER(_Info)]),
         "fann_set_timing": (i, [p, i]),
         "fann_last_timing": (i, [p] + [C.POINTER(C.c_float)] * 4),
+        "fann_gather_probe": (i, [p, p, u64, p, p]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -175,7 +178,11 @@ def fann_set_timing(ix, enable: bool) -> None:
 def fann_last_timing(ix) -> dict:
     v = [C.c_float(-1.0) for _ in range(4)]
     _check(load_library().fann_last_timing(ix, *[C.byref(x) for x in v]))
-    return dict(zip(("lut_ms", "plan_ms", "scan_ms", "merge_ms"), (float(x.value) for x in v)))
+    return dict(zip(("lut_ms", "plan_ms", "dedup_ms", "scan_ms"), (float(x.value) for x in v)))
+
+
+def fann_gather_probe(ix, ids, n, sink, stream=None) -> None:
+    _check(load_library().fann_gather_probe(ix, _addr(ids), n, _addr(sink), stream))
 
 
 # ---- convenience wrapper (torch for device memory and streams only) ----------

@@ -19,17 +19,21 @@ struct fann_index {
     size_t bounce_bytes = 0;
     int num_sms = 0;
     int smem_optin = 0;                    // max dynamic shared memory per block
-    uint32_t ipt = 2;                      // candidate IDs per thread per block-synchronous step
+    uint32_t chunks = 1;                   // batch chunks: dedup of chunk i+1 runs beside the scan of chunk i
+    uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint64_t launches = 0;
-    // geometry of the last scan launch (fann_get_info)
-    uint32_t last_ctas = 0, last_smem = 0, last_slots = 0;
-    // optional per-kernel timing: events 0/1 lut, 2/3 plan, 3/4 scan, 4/5 merge
+    // second stream + events for the dedup/scan overlap
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_dedup_done[kMaxChunks] = {}, ev_join = nullptr;
+    // geometry of the last launches (fann_get_info)
+    uint32_t last_dedup_ctas = 0, last_scan_ctas = 0, last_scan_smem = 0, last_cap = 0, last_slots = 0, last_chunks = 0;
+    // optional per-kernel timing
     bool timing = false;
-    cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    bool ev_lut = false, ev_scan = false, ev_merge = false;
+    cudaEvent_t ev_lut[2] = {}, ev_plan[2] = {}, ev_dedup[kMaxChunks][2] = {}, ev_scan[kMaxChunks][2] = {};
+    bool have_lut = false, have_scan = false;
+    uint32_t timed_chunks = 0;
+    bool timed_scan = false;
 };
-
-static inline void rec(fann_index *ix, int i, cudaStream_t s) { if (ix->timing) cudaEventRecord(ix->ev[i], s); }
 
 static thread_local char g_err[512] = "";
 
@@ -56,66 +60,52 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
-static uint32_t next_pow2(uint32_t v)
-{
-    uint32_t p = 1;
-    while (p < v) p <<= 1;
-    return p;
-}
-
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // ---------------------------------------------------------------- geometry + workspace layout
 
-struct ScanGeom {
-    uint32_t KP, capbuf, ipt, nslots, cap_c, smem_bytes;
+struct Geom {
+    uint32_t nslots_max, cap_c, dedup_smem;          // dedup: table slots per CTA, candidates per partition
+    uint32_t cap, scan_smem;                         // scan: candidate-buffer keys, shared memory per CTA
 };
 
-static int scan_geometry(const fann_index *ix, uint32_t k, ScanGeom *g)
+static void geometry(const fann_index *ix, uint32_t k, Geom *g)
 {
-    g->ipt = ix->ipt;
-    g->KP = next_pow2(k < 32 ? 32 : k);
-    g->capbuf = next_pow2(k + kScanThreads * (g->ipt + 1));
-    const size_t fixed = scan_smem_bytes(g->capbuf, ix->row_bytes, 0);
-    if (fixed + 4096 * 4 > (size_t)ix->smem_optin)
-        return fail(FANN_EUNSUPPORTED, "shared memory: %zu bytes fixed + table > %d", fixed, ix->smem_optin);
-    g->nslots = (uint32_t)(((size_t)ix->smem_optin - fixed) / 4) & ~3u;
-    g->cap_c = (uint32_t)((uint64_t)g->nslots * 4 / 5);          // <= 80 % load even with no repeats
-    g->smem_bytes = (uint32_t)scan_smem_bytes(g->capbuf, ix->row_bytes, g->nslots);
-    return FANN_OK;
+    g->dedup_smem = ix->dedup_smem;
+    g->nslots_max = ((g->dedup_smem - 64) / 4) & ~3u;
+    g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
+    g->cap = k <= 256 ? 4096u : 8192u;
+    g->scan_smem = (uint32_t)scan_smem_bytes(g->cap);
 }
 
 struct WsLayout {
-    size_t hdr, S, item_start, items, part_count, part_uniq, part_keys, total;
+    size_t hdr, S, item_start, items, uniq_counts, uniq_ids, total;
     uint32_t max_items;
 };
 
-static void ws_layout(uint32_t B, uint64_t total_cands, const ScanGeom &g, WsLayout *w)
+static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with_uniq, WsLayout *w)
 {
     const uint64_t max_items = (uint64_t)B + total_cands / g.cap_c + 1;
     w->max_items = (uint32_t)(max_items > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : max_items);
     size_t o = 0;
-    w->hdr = o;        o = align_up(o + 256, 256);
-    w->S = o;          o = align_up(o + (size_t)B * 4, 256);
-    w->item_start = o; o = align_up(o + ((size_t)B + 1) * 4, 256);
-    w->items = o;      o = align_up(o + (size_t)w->max_items * 8, 256);
-    w->part_count = o; o = align_up(o + (size_t)w->max_items * 4, 256);
-    w->part_uniq = o;  o = align_up(o + (size_t)w->max_items * 4, 256);
-    w->part_keys = o;  o = align_up(o + (size_t)w->max_items * g.KP * 8, 256);
+    w->hdr = o;         o = align_up(o + 256, 256);
+    w->S = o;           o = align_up(o + (size_t)B * 4, 256);
+    w->item_start = o;  o = align_up(o + ((size_t)B + 1) * 4, 256);
+    w->items = o;       o = align_up(o + (size_t)w->max_items * 8, 256);
+    w->uniq_counts = o; o = align_up(o + (size_t)B * 4, 256);
+    w->uniq_ids = o;    if (with_uniq) o = align_up(o + (size_t)total_cands * 4 + 16, 256);
     w->total = o;
 }
 
 // ---------------------------------------------------------------- lifecycle
 
 extern "C" const char *fann_last_error(void) { return g_err; }
-extern "C" const char *fann_version(void) { return "fann 0.1 sm_100a"; }
+extern "C" const char *fann_version(void) { return "fann 0.2 sm_100a"; }
 
-template <int NCHUNK>
-static cudaError_t set_scan_attrs(int smem)
+template <int G, int NB>
+static cudaError_t set_scan_attr(int smem)
 {
-    cudaError_t e = cudaFuncSetAttribute(scan_kernel<NCHUNK, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(scan_kernel<NCHUNK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    return cudaFuncSetAttribute(scan_kernel<G, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
 extern "C" int fann_create(fann_index **out, int device)
@@ -132,13 +122,26 @@ extern "C" int fann_create(fann_index **out, int device)
     int num_sms = 0, smem_optin = 0;
     CUDA_TRY(cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, device));
     CUDA_TRY(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device));
-    CUDA_TRY(set_scan_attrs<1>(smem_optin));
-    CUDA_TRY(set_scan_attrs<2>(smem_optin));
-    CUDA_TRY(set_scan_attrs<3>(smem_optin));
-    CUDA_TRY(set_scan_attrs<4>(smem_optin));
+    const int scan_max = (int)scan_smem_bytes(8192);
+    if (scan_max > smem_optin)
+        return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
+                    smem_optin, scan_max);
+    CUDA_TRY(cudaFuncSetAttribute(dedup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
+    CUDA_TRY((set_scan_attr<1, 4>(scan_max)));
+    CUDA_TRY((set_scan_attr<2, 4>(scan_max)));
+    CUDA_TRY((set_scan_attr<4, 2>(scan_max)));
     fann_index *ix = new fann_index();
     ix->device = device; ix->num_sms = num_sms; ix->smem_optin = smem_optin;
-    if (const char *s = getenv("FANN_IPT")) { int v = atoi(s); if (v >= 1 && v <= 4) ix->ipt = (uint32_t)v; }
+    ix->dedup_smem = (uint32_t)smem_optin;
+    if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
+    if (const char *s = getenv("FANN_DEDUP_SMEM_KB")) {
+        int v = atoi(s) * 1024;
+        if (v >= 16 * 1024 && v <= smem_optin) ix->dedup_smem = (uint32_t)v;
+    }
+    CUDA_TRY(cudaStreamCreateWithFlags(&ix->side, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&ix->ev_fork, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventCreateWithFlags(&ix->ev_join, cudaEventDisableTiming));
+    for (auto &ev : ix->ev_dedup_done) CUDA_TRY(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
     *out = ix;
     return FANN_OK;
 }
@@ -150,7 +153,14 @@ extern "C" void fann_destroy(fann_index *ix)
     cudaDeviceSynchronize();
     if (ix->codes) cudaFree(ix->codes);
     if (ix->bounce) cudaFree(ix->bounce);
-    for (auto &e : ix->ev) if (e) cudaEventDestroy(e);
+    if (ix->side) cudaStreamDestroy(ix->side);
+    if (ix->ev_fork) cudaEventDestroy(ix->ev_fork);
+    if (ix->ev_join) cudaEventDestroy(ix->ev_join);
+    for (auto &e : ix->ev_dedup_done) if (e) cudaEventDestroy(e);
+    for (auto &e : ix->ev_lut) if (e) cudaEventDestroy(e);
+    for (auto &e : ix->ev_plan) if (e) cudaEventDestroy(e);
+    for (auto &c : ix->ev_dedup) for (auto &e : c) if (e) cudaEventDestroy(e);
+    for (auto &c : ix->ev_scan) for (auto &e : c) if (e) cudaEventDestroy(e);
     delete ix;
 }
 
@@ -158,13 +168,19 @@ extern "C" int fann_get_info(const fann_index *ix, fann_info *out)
 {
     if (!ix || !out) return fail(FANN_EINVAL, "fann_get_info: NULL argument");
     out->N = ix->N; out->M = ix->M; out->row_bytes = ix->row_bytes;
-    out->num_sms = (uint32_t)ix->num_sms; out->scan_threads = kScanThreads;
-    out->scan_ctas = ix->last_ctas; out->scan_smem_bytes = ix->last_smem; out->table_slots = ix->last_slots;
+    out->num_sms = (uint32_t)ix->num_sms;
+    out->dedup_threads = kDedupThreads; out->dedup_ctas = ix->last_dedup_ctas;
+    out->dedup_smem_bytes = ix->dedup_smem; out->table_slots = ix->last_slots;
+    out->scan_threads = kScanThreads; out->scan_ctas = ix->last_scan_ctas;
+    out->scan_smem_bytes = ix->last_scan_smem; out->scan_buffer_keys = ix->last_cap;
+    out->chunks = ix->last_chunks;
     out->kernel_launches = ix->launches;
     return FANN_OK;
 }
 
 // ---------------------------------------------------------------- fann_load_codes
+
+static uint32_t stored_row_bytes(uint32_t M) { return M <= 16 ? 16u : (M <= 32 ? 32u : 64u); }
 
 extern "C" int fann_load_codes(fann_index *ix, const uint8_t *codes, uint64_t first, uint64_t n,
                                uint64_t N_total, uint32_t M, int src_is_device, void *stream_)
@@ -178,7 +194,7 @@ extern "C" int fann_load_codes(fann_index *ix, const uint8_t *codes, uint64_t fi
     DeviceGuard guard(ix->device);
     cudaStream_t stream = (cudaStream_t)stream_;
     if (!ix->codes) {
-        ix->N = N_total; ix->M = M; ix->row_bytes = (M + 15u) & ~15u;
+        ix->N = N_total; ix->M = M; ix->row_bytes = stored_row_bytes(M);
         cudaError_t e = cudaMalloc(&ix->codes, (size_t)N_total * ix->row_bytes);
         if (e != cudaSuccess) {
             ix->codes = nullptr; ix->N = 0; ix->M = 0;
@@ -242,12 +258,11 @@ extern "C" int fann_build_lut(fann_index *ix, const float *queries, uint32_t B,
     if (B == 0) return fail(FANN_EINVAL, "fann_build_lut: B == 0");
     if (dsub == 0 || dsub > 64) return fail(FANN_EUNSUPPORTED, "fann_build_lut: dsub=%u not in 1..64", dsub);
     DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
     const uint64_t units = (uint64_t)B * ix->M * 64;
-    rec(ix, 0, (cudaStream_t)stream_);
-    build_lut_kernel<<<(unsigned)((units + 255) / 256), 256, 0, (cudaStream_t)stream_>>>(
-        queries, codebooks, lut, B, ix->M, dsub);
-    rec(ix, 1, (cudaStream_t)stream_);
-    ix->ev_lut = ix->timing;
+    if (ix->timing) cudaEventRecord(ix->ev_lut[0], stream);
+    build_lut_kernel<<<(unsigned)((units + 255) / 256), 256, 0, stream>>>(queries, codebooks, lut, B, ix->M, dsub);
+    if (ix->timing) { cudaEventRecord(ix->ev_lut[1], stream); ix->have_lut = true; }
     ix->launches++;
     CUDA_TRY(cudaGetLastError());
     return FANN_OK;
@@ -259,36 +274,48 @@ extern "C" size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_
 {
     if (!ix || !ix->codes) { fail(FANN_EINVAL, "fann_workspace_bytes: index has no codes"); return 0; }
     if (B == 0 || k == 0 || k > FANN_MAX_K) { fail(FANN_EINVAL, "fann_workspace_bytes: B=%u k=%u", B, k); return 0; }
-    ScanGeom g;
-    if (scan_geometry(ix, k, &g) != FANN_OK) return 0;
+    Geom g;
+    geometry(ix, k, &g);
     WsLayout w;
-    ws_layout(B, total_cands, g, &w);
+    ws_layout(B, total_cands, g, true, &w);
     return w.total;
 }
 
-template <bool DUMP>
-static cudaError_t launch_scan(uint32_t nchunk, int grid, size_t smem, cudaStream_t stream, const ScanParams &p)
+static cudaError_t launch_scan(const fann_index *ix, int grid, size_t smem, cudaStream_t stream, const ScanParams &p)
 {
-    switch (nchunk) {
-    case 1: scan_kernel<1, DUMP><<<grid, kScanThreads, smem, stream>>>(p); break;
-    case 2: scan_kernel<2, DUMP><<<grid, kScanThreads, smem, stream>>>(p); break;
-    case 3: scan_kernel<3, DUMP><<<grid, kScanThreads, smem, stream>>>(p); break;
-    default: scan_kernel<4, DUMP><<<grid, kScanThreads, smem, stream>>>(p); break;
+    switch (ix->row_bytes) {
+    case 16: scan_kernel<1, 4><<<grid, kScanThreads, smem, stream>>>(p); break;
+    case 32: scan_kernel<2, 4><<<grid, kScanThreads, smem, stream>>>(p); break;
+    default: scan_kernel<4, 2><<<grid, kScanThreads, smem, stream>>>(p); break;
     }
     return cudaGetLastError();
 }
 
-static int run_scan(fann_index *ix, bool dump, const float *lut, uint32_t B,
+static int scan_ctas_per_sm(const fann_index *ix, size_t smem)
+{
+    int n = 0;
+    cudaError_t e;
+    switch (ix->row_bytes) {
+    case 16: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<1, 4>, kScanThreads, smem); break;
+    case 32: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<2, 4>, kScanThreads, smem); break;
+    default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<4, 2>, kScanThreads, smem); break;
+    }
+    return (e == cudaSuccess && n >= 1) ? n : 1;
+}
+
+// plan + dedup (+ scan unless dump).  With chunks > 1 the dedup launches go to the index's side
+// stream and the scan of chunk i waits only for the dedup of chunk i, so the HBM-bound scan and
+// the shared-memory-bound dedup of the next chunk share the SMs.
+static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     const int64_t *cand_offsets, const uint32_t *cand_ids, uint64_t total_cands,
                     uint32_t k, uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
                     uint32_t *out_uniq, uint32_t *uniq_ids, uint32_t *uniq_counts,
                     void *workspace, size_t workspace_bytes, cudaStream_t stream)
 {
-    ScanGeom g;
-    int rc = scan_geometry(ix, k, &g);
-    if (rc != FANN_OK) return rc;
+    Geom g;
+    geometry(ix, k, &g);
     WsLayout w;
-    ws_layout(B, total_cands, g, &w);
+    ws_layout(B, total_cands, g, !dump, &w);
     if (!workspace || ((uintptr_t)workspace & 255) != 0)
         return fail(FANN_EWORKSPACE, "workspace is NULL or not 256-byte aligned");
     if (workspace_bytes < w.total)
@@ -299,39 +326,68 @@ static int run_scan(fann_index *ix, bool dump, const float *lut, uint32_t B,
     uint32_t *S = (uint32_t *)(ws + w.S);
     uint32_t *item_start = (uint32_t *)(ws + w.item_start);
     uint2 *items = (uint2 *)(ws + w.items);
+    if (!dump) { uniq_counts = (uint32_t *)(ws + w.uniq_counts); uniq_ids = (uint32_t *)(ws + w.uniq_ids); }
 
-    rec(ix, 2, stream);
+    const bool timing = ix->timing;
+    if (timing) cudaEventRecord(ix->ev_plan[0], stream);
     plan_kernel<<<1, 1024, 0, stream>>>((const long long *)cand_offsets, B, g.cap_c, w.max_items, hdr, S,
-                                        item_start, items, dump ? uniq_counts : nullptr);
+                                        item_start, items, uniq_counts);
+    if (timing) cudaEventRecord(ix->ev_plan[1], stream);
     ix->launches++;
     CUDA_TRY(cudaGetLastError());
 
-    ScanParams p;
-    p.codes = ix->codes; p.N = ix->N; p.row_bytes = ix->row_bytes; p.lut = lut; p.M = ix->M;
-    p.cand_offsets = (const long long *)cand_offsets; p.cand_ids = cand_ids;
-    p.k = k; p.KP = g.KP; p.capbuf = g.capbuf; p.ipt = g.ipt; p.nslots = g.nslots;
-    p.hdr = hdr; p.S = S; p.items = items;
-    p.part_count = (uint32_t *)(ws + w.part_count);
-    p.part_uniq = (uint32_t *)(ws + w.part_uniq);
-    p.part_keys = (unsigned long long *)(ws + w.part_keys);
-    p.uniq_ids = uniq_ids; p.uniq_counts = uniq_counts;
-    const int grid = ix->num_sms;                                   // persistent: one CTA per SM
-    rec(ix, 3, stream);
-    cudaError_t e = dump ? launch_scan<true>(ix->row_bytes >> 4, grid, g.smem_bytes, stream, p)
-                         : launch_scan<false>(ix->row_bytes >> 4, grid, g.smem_bytes, stream, p);
-    ix->launches++;
-    if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
-    ix->last_ctas = (uint32_t)grid; ix->last_smem = g.smem_bytes; ix->last_slots = g.nslots;
-    rec(ix, 4, stream);
-    ix->ev_scan = ix->timing; ix->ev_merge = false;
-    if (!dump) {
-        merge_kernel<<<B, 256, (size_t)2 * g.KP * 8, stream>>>(k, g.KP, hdr, S, item_start, p.part_uniq,
-                                                               p.part_keys, out_ids, out_dists, out_counts, out_uniq);
-        rec(ix, 5, stream);
-        ix->ev_merge = ix->timing;
+    uint32_t chunks = dump ? 1u : ix->chunks;
+    if (chunks > B) chunks = B;
+    const bool overlap = chunks > 1;
+    cudaStream_t dstream = overlap ? ix->side : stream;
+    if (overlap) {
+        CUDA_TRY(cudaEventRecord(ix->ev_fork, stream));
+        CUDA_TRY(cudaStreamWaitEvent(ix->side, ix->ev_fork, 0));
+    }
+
+    DedupParams dp;
+    dp.cand_offsets = (const long long *)cand_offsets; dp.cand_ids = cand_ids; dp.N = ix->N;
+    dp.nslots_max = g.nslots_max; dp.hdr = hdr; dp.S = S; dp.item_start = item_start; dp.items = items;
+    dp.uniq_ids = uniq_ids; dp.uniq_counts = uniq_counts;
+    ScanParams sp;
+    sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
+    sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
+    sp.out_ids = out_ids; sp.out_dists = out_dists; sp.out_counts = out_counts; sp.out_uniq = out_uniq;
+    const int per_sm = dump ? 1 : scan_ctas_per_sm(ix, g.scan_smem);
+
+    for (uint32_t c = 0; c < chunks; ++c) {
+        const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
+        dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
+        if (timing) cudaEventRecord(ix->ev_dedup[c][0], dstream);
+        dedup_kernel<<<ix->num_sms, kDedupThreads, g.dedup_smem, dstream>>>(dp);
+        if (timing) cudaEventRecord(ix->ev_dedup[c][1], dstream);
         ix->launches++;
         CUDA_TRY(cudaGetLastError());
+        if (overlap) CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], dstream));
     }
+    ix->last_dedup_ctas = (uint32_t)ix->num_sms; ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
+    ix->timed_chunks = timing ? chunks : 0; ix->timed_scan = false;
+    if (!dump) {
+        for (uint32_t c = 0; c < chunks; ++c) {
+            const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
+            sp.q_begin = qb; sp.q_end = qe; sp.counter = &hdr->scan_counter[c];
+            int grid = ix->num_sms * per_sm;
+            if ((uint32_t)grid > qe - qb) grid = (int)(qe - qb);
+            if (overlap) CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_dedup_done[c], 0));
+            if (timing) cudaEventRecord(ix->ev_scan[c][0], stream);
+            cudaError_t e = launch_scan(ix, grid, g.scan_smem, stream, sp);
+            if (timing) cudaEventRecord(ix->ev_scan[c][1], stream);
+            ix->launches++;
+            if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
+            ix->last_scan_ctas = (uint32_t)grid;
+        }
+        ix->last_scan_smem = g.scan_smem; ix->last_cap = g.cap;
+        ix->timed_scan = timing;
+    } else if (overlap) {
+        CUDA_TRY(cudaEventRecord(ix->ev_join, dstream));
+        CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_join, 0));
+    }
+    ix->have_scan = timing;
     return FANN_OK;
 }
 
@@ -348,7 +404,7 @@ extern "C" int fann_dedup_scan_topk(fann_index *ix, const float *lut, uint32_t B
     if (!ix->codes) return fail(FANN_EINVAL, "fann_dedup_scan_topk: load codes first");
     if (B == 0) return fail(FANN_EINVAL, "fann_dedup_scan_topk: B == 0");
     if (k == 0 || k > FANN_MAX_K) return fail(FANN_EUNSUPPORTED, "fann_dedup_scan_topk: k=%u not in 1..%u", k, FANN_MAX_K);
-    return run_scan(ix, false, lut, B, cand_offsets, cand_ids, total_cands, k, out_ids, out_dists,
+    return run_path(ix, false, lut, B, cand_offsets, cand_ids, total_cands, k, out_ids, out_dists,
                     out_counts, out_uniq, nullptr, nullptr, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
@@ -361,7 +417,7 @@ extern "C" int fann_dedup_only(fann_index *ix, uint32_t B, const int64_t *cand_o
     if ((!cand_ids || !uniq_ids) && total_cands) return fail(FANN_EINVAL, "fann_dedup_only: NULL id array");
     if (!ix->codes) return fail(FANN_EINVAL, "fann_dedup_only: load codes first (N is unknown)");
     if (B == 0) return fail(FANN_EINVAL, "fann_dedup_only: B == 0");
-    return run_scan(ix, true, nullptr, B, cand_offsets, cand_ids, total_cands, 1, nullptr, nullptr,
+    return run_path(ix, true, nullptr, B, cand_offsets, cand_ids, total_cands, 1, nullptr, nullptr,
                     nullptr, nullptr, uniq_ids, uniq_counts, workspace, workspace_bytes, (cudaStream_t)stream);
 }
 
@@ -385,14 +441,13 @@ struct HostScratch {
     size_t queries, offsets, ids, lut, out_ids, out_dists, out_counts, ws, ws_bytes, total;
 };
 
-static int host_scratch_layout(const fann_index *ix, uint32_t B, uint32_t dsub, uint64_t total_cands,
-                               uint32_t k, HostScratch *h)
+static void host_scratch_layout(const fann_index *ix, uint32_t B, uint32_t dsub, uint64_t total_cands,
+                                uint32_t k, HostScratch *h)
 {
-    ScanGeom g;
-    int rc = scan_geometry(ix, k, &g);
-    if (rc != FANN_OK) return rc;
+    Geom g;
+    geometry(ix, k, &g);
     WsLayout w;
-    ws_layout(B, total_cands, g, &w);
+    ws_layout(B, total_cands, g, true, &w);
     size_t o = 0;
     h->queries = o;    o = align_up(o + (size_t)B * ix->M * dsub * 4, 256);
     h->offsets = o;    o = align_up(o + ((size_t)B + 1) * 8, 256);
@@ -403,7 +458,6 @@ static int host_scratch_layout(const fann_index *ix, uint32_t B, uint32_t dsub, 
     h->out_counts = o; o = align_up(o + (size_t)B * 4, 256);
     h->ws = o;         h->ws_bytes = w.total; o += w.total;
     h->total = o;
-    return FANN_OK;
 }
 
 extern "C" size_t fann_search_host_scratch_bytes(const fann_index *ix, uint32_t B, uint32_t dsub,
@@ -414,7 +468,7 @@ extern "C" size_t fann_search_host_scratch_bytes(const fann_index *ix, uint32_t 
         return 0;
     }
     HostScratch h;
-    if (host_scratch_layout(ix, B, dsub, total_cands, k, &h) != FANN_OK) return 0;
+    host_scratch_layout(ix, B, dsub, total_cands, k, &h);
     return h.total;
 }
 
@@ -432,8 +486,7 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
     const uint64_t total = (uint64_t)cand_offsets_h[B];
     if (!cand_ids_h && total) return fail(FANN_EINVAL, "fann_search_host: cand_ids_h is NULL");
     HostScratch h;
-    int rc = host_scratch_layout(ix, B, dsub, total, k, &h);
-    if (rc != FANN_OK) return rc;
+    host_scratch_layout(ix, B, dsub, total, k, &h);
     if (!device_scratch || ((uintptr_t)device_scratch & 255) != 0 || scratch_bytes < h.total)
         return fail(FANN_EWORKSPACE, "fann_search_host: scratch has %zu bytes, %zu needed (256-byte aligned)",
                     scratch_bytes, h.total);
@@ -444,7 +497,7 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
     CUDA_TRY(cudaMemcpyAsync(s + h.offsets, cand_offsets_h, ((size_t)B + 1) * 8, cudaMemcpyHostToDevice, stream));
     if (total)
         CUDA_TRY(cudaMemcpyAsync(s + h.ids, cand_ids_h, (size_t)total * 4, cudaMemcpyHostToDevice, stream));
-    rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
+    int rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
     if (rc != FANN_OK) return rc;
     rc = fann_dedup_scan_topk(ix, (const float *)(s + h.lut), B, (const int64_t *)(s + h.offsets),
                               (const uint32_t *)(s + h.ids), total, k, (uint32_t *)(s + h.out_ids),
@@ -459,35 +512,70 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
     return fann_workspace_status(ix, s + h.ws, stream);
 }
 
-// ---------------------------------------------------------------- timing
+// ---------------------------------------------------------------- measurement
+
+extern "C" int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink, void *stream_)
+{
+    if (!ix || !ids || !sink) return fail(FANN_EINVAL, "fann_gather_probe: NULL argument");
+    if (!ix->codes) return fail(FANN_EINVAL, "fann_gather_probe: load codes first");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const int grid = ix->num_sms * 2;
+    switch (ix->row_bytes) {
+    case 16: gather_probe_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink); break;
+    case 32: gather_probe_kernel<2, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink); break;
+    default: gather_probe_kernel<4, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink); break;
+    }
+    ix->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return FANN_OK;
+}
 
 extern "C" int fann_set_timing(fann_index *ix, int enable)
 {
     if (!ix) return fail(FANN_EINVAL, "fann_set_timing: NULL index");
     DeviceGuard guard(ix->device);
-    if (enable)
-        for (auto &e : ix->ev)
-            if (!e) CUDA_TRY(cudaEventCreate(&e));
+    if (enable) {
+        for (auto &e : ix->ev_lut) if (!e) CUDA_TRY(cudaEventCreate(&e));
+        for (auto &e : ix->ev_plan) if (!e) CUDA_TRY(cudaEventCreate(&e));
+        for (auto &c : ix->ev_dedup) for (auto &e : c) if (!e) CUDA_TRY(cudaEventCreate(&e));
+        for (auto &c : ix->ev_scan) for (auto &e : c) if (!e) CUDA_TRY(cudaEventCreate(&e));
+    }
     ix->timing = enable != 0;
-    ix->ev_lut = ix->ev_scan = ix->ev_merge = false;
+    ix->have_lut = ix->have_scan = false;
+    ix->timed_chunks = 0; ix->timed_scan = false;
     return FANN_OK;
 }
 
-extern "C" int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *scan_ms, float *merge_ms)
+extern "C" int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup_ms, float *scan_ms)
 {
     if (!ix) return fail(FANN_EINVAL, "fann_last_timing: NULL index");
     DeviceGuard guard(ix->device);
     float v[4] = {-1.f, -1.f, -1.f, -1.f};
-    if (ix->ev_lut) { CUDA_TRY(cudaEventSynchronize(ix->ev[1])); CUDA_TRY(cudaEventElapsedTime(&v[0], ix->ev[0], ix->ev[1])); }
-    if (ix->ev_scan) {
-        CUDA_TRY(cudaEventSynchronize(ix->ev[4]));
-        CUDA_TRY(cudaEventElapsedTime(&v[1], ix->ev[2], ix->ev[3]));
-        CUDA_TRY(cudaEventElapsedTime(&v[2], ix->ev[3], ix->ev[4]));
+    if (ix->have_lut) { CUDA_TRY(cudaEventSynchronize(ix->ev_lut[1])); CUDA_TRY(cudaEventElapsedTime(&v[0], ix->ev_lut[0], ix->ev_lut[1])); }
+    if (ix->have_scan && ix->timed_chunks) {
+        CUDA_TRY(cudaEventSynchronize(ix->ev_plan[1]));
+        CUDA_TRY(cudaEventElapsedTime(&v[1], ix->ev_plan[0], ix->ev_plan[1]));
+        v[2] = 0.f;
+        for (uint32_t c = 0; c < ix->timed_chunks; ++c) {
+            float t = 0.f;
+            CUDA_TRY(cudaEventSynchronize(ix->ev_dedup[c][1]));
+            CUDA_TRY(cudaEventElapsedTime(&t, ix->ev_dedup[c][0], ix->ev_dedup[c][1]));
+            v[2] += t;
+        }
+        if (ix->timed_scan) {
+            v[3] = 0.f;
+            for (uint32_t c = 0; c < ix->timed_chunks; ++c) {
+                float t = 0.f;
+                CUDA_TRY(cudaEventSynchronize(ix->ev_scan[c][1]));
+                CUDA_TRY(cudaEventElapsedTime(&t, ix->ev_scan[c][0], ix->ev_scan[c][1]));
+                v[3] += t;
+            }
+        }
     }
-    if (ix->ev_merge) { CUDA_TRY(cudaEventSynchronize(ix->ev[5])); CUDA_TRY(cudaEventElapsedTime(&v[3], ix->ev[4], ix->ev[5])); }
     if (lut_ms) *lut_ms = v[0];
     if (plan_ms) *plan_ms = v[1];
-    if (scan_ms) *scan_ms = v[2];
-    if (merge_ms) *merge_ms = v[3];
+    if (dedup_ms) *dedup_ms = v[2];
+    if (scan_ms) *scan_ms = v[3];
     return FANN_OK;
 }
