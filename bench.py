@@ -117,6 +117,8 @@ def main():
     ap.add_argument("--cpu-queries", type=int, default=0, help="oracle sample size (0 = auto, ~10-30 s)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--scale-N", type=int, default=0, help="profiling only: same per-query shape on N vectors")
+    ap.add_argument("--scale-B", type=int, default=0, help="profiling only: batch of B queries")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -128,6 +130,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     cfg = CONFIGS[args.workload]
+    if args.scale_N or args.scale_B:                 # scaled copies are for ncu captures, never a bench value
+        N = args.scale_N or cfg.N
+        cfg = cfg.scaled(name=f"{cfg.name}@N={N},B={args.scale_B or cfg.B}", N=N, B=args.scale_B or cfg.B,
+                         n_lists=max(4 * cfg.nprobe, cfg.n_lists * N // cfg.N))
 
     if args.impl == "reference":
         return reference_arm(args, cfg, rank, world)

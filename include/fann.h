@@ -211,7 +211,8 @@ int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup
  * ceiling of step (6).  IDs >= N read row 0.
  * ids  device, [n] uint32      sink  device, 4 bytes (never written in practice)
  */
-int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink, void *stream);
+int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink,
+                      uint32_t flavor, void *stream);
 
 #ifdef __cplusplus
 }

@@ -69,7 +69,7 @@ def load_library():
         "fann_get_info": (i, [p, C.POINTER(_Info)]),
         "fann_set_timing": (i, [p, i]),
         "fann_last_timing": (i, [p] + [C.POINTER(C.c_float)] * 4),
-        "fann_gather_probe": (i, [p, p, u64, p, p]),
+        "fann_gather_probe": (i, [p, p, u64, p, u32, p]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -181,8 +181,8 @@ def fann_last_timing(ix) -> dict:
     return dict(zip(("lut_ms", "plan_ms", "dedup_ms", "scan_ms"), (float(x.value) for x in v)))
 
 
-def fann_gather_probe(ix, ids, n, sink, stream=None) -> None:
-    _check(load_library().fann_gather_probe(ix, _addr(ids), n, _addr(sink), stream))
+def fann_gather_probe(ix, ids, n, sink, flavor=0, stream=None) -> None:
+    _check(load_library().fann_gather_probe(ix, _addr(ids), n, _addr(sink), flavor, stream))
 
 
 # ---- convenience wrapper (torch for device memory and streams only) ----------

@@ -134,6 +134,10 @@ extern "C" int fann_create(fann_index **out, int device)
     ix->device = device; ix->num_sms = num_sms; ix->smem_optin = smem_optin;
     ix->dedup_smem = (uint32_t)smem_optin;
     if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
+    if (const char *s = getenv("FANN_L2_FETCH")) {
+        int v = atoi(s);
+        if (v == 32 || v == 64 || v == 128) CUDA_TRY(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)v));
+    }
     if (const char *s = getenv("FANN_DEDUP_SMEM_KB")) {
         int v = atoi(s) * 1024;
         if (v >= 16 * 1024 && v <= smem_optin) ix->dedup_smem = (uint32_t)v;
@@ -514,17 +518,23 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
 
 // ---------------------------------------------------------------- measurement
 
-extern "C" int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink, void *stream_)
+extern "C" int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink,
+                                 uint32_t flavor, void *stream_)
 {
     if (!ix || !ids || !sink) return fail(FANN_EINVAL, "fann_gather_probe: NULL argument");
     if (!ix->codes) return fail(FANN_EINVAL, "fann_gather_probe: load codes first");
+    if (flavor > 7) return fail(FANN_EINVAL, "fann_gather_probe: flavor %u not in 0..7", flavor);
+    if (flavor >= 6 && ix->row_bytes < 32) return fail(FANN_EUNSUPPORTED, "fann_gather_probe: 32-byte loads need rows >= 32 bytes");
     DeviceGuard guard(ix->device);
     cudaStream_t stream = (cudaStream_t)stream_;
     const int grid = ix->num_sms * 2;
-    switch (ix->row_bytes) {
-    case 16: gather_probe_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink); break;
-    case 32: gather_probe_kernel<2, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink); break;
-    default: gather_probe_kernel<4, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink); break;
+    if (flavor >= 6) {
+        if (ix->row_bytes == 32) gather_probe256_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor);
+        else gather_probe256_kernel<2, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor);
+    } else switch (ix->row_bytes) {
+    case 16: gather_probe_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor); break;
+    case 32: gather_probe_kernel<2, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor); break;
+    default: gather_probe_kernel<4, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor); break;
     }
     ix->launches++;
     CUDA_TRY(cudaGetLastError());

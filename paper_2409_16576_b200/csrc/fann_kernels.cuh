@@ -188,14 +188,34 @@ struct DedupParams {
     uint32_t *uniq_counts;                           // [B], zeroed by plan_kernel
 };
 
-// PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm": open addressing with
-// linear probing in shared memory; a slot is claimed with atomicCAS (no spinlock).  Each CTA pass
-// handles the IDs of one query that hash into one partition, then compacts its table into the
-// query's distinct list (order arbitrary).
+// Elements e0 .. e0+3 of a candidate list of C IDs (e0 may be negative or reach past the end at the
+// two ragged ends of a list); positions outside [0, C) read as kIdNone.  ids + e0 is 16-byte aligned.
+__device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, uint32_t C)
+{
+    if (e0 >= 0 && e0 + 3 < (long long)C) return __ldg(reinterpret_cast<const uint4 *>(ids + e0));
+    uint4 r = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+    if (e0 >= 0 && e0 < (long long)C) r.x = __ldg(ids + e0);
+    if (e0 + 1 >= 0 && e0 + 1 < (long long)C) r.y = __ldg(ids + e0 + 1);
+    if (e0 + 2 >= 0 && e0 + 2 < (long long)C) r.z = __ldg(ids + e0 + 2);
+    if (e0 + 3 >= 0 && e0 + 3 < (long long)C) r.w = __ldg(ids + e0 + 3);
+    return r;
+}
+
+// PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel
+// takes a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-
+// memory pipe on this part.  This kernel uses neither: open addressing with linear probing in shared
+// memory, advanced in CTA-wide rounds of a READ phase and a WRITE phase with a barrier after each.
+// Read phase: every pending ID reads its slot -- equal: done (a repeat, or its own store of the last
+// write phase survived); another ID: next slot; empty: store it in the write phase and look again.
+// No store is in flight during a read phase, so a slot seen non-empty keeps its value for good and
+// may be skipped safely; of several stores to one empty slot one survives and the losers see that in
+// the next read phase.  All copies of an ID walk the same probe sequence, so exactly one slot ends up
+// holding it.  Each CTA pass handles the IDs of one query that hash into one partition, then compacts
+// its table into the query's distinct list (order arbitrary).
 __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupParams p)
 {
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] winners [2] out base [3] write pos
+    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] distinct here [2] out base [3] write pos
     uint32_t *table = reinterpret_cast<uint32_t *>(smem + 64);
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     const uint32_t lt_mask = (1u << lane) - 1u;
@@ -227,61 +247,82 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
         }
         __syncthreads();
 
-        uint32_t won = 0;
-        auto insert = [&](uint32_t id) {
-            if (id == kIdNone || (uint64_t)id >= p.N) return;
-            uint32_t a = (id ^ (id >> 16)) * 0x7feb352dU;
-            if (S > 1 && __umulhi(a, S) != part) return;
-            a = (a ^ (a >> 15)) * 0x846ca68bU;
-            a ^= a >> 16;
-            uint32_t slot = __umulhi(a, nslots);
-            for (uint32_t probes = 0;; ++probes) {
-                const uint32_t cur = *reinterpret_cast<volatile uint32_t *>(table + slot);
-                if (cur == id) return;
-                if (cur == kEmpty) {
-                    const uint32_t old = atomicCAS(table + slot, kEmpty, id);
-                    if (old == kEmpty) { ++won; return; }
-                    if (old == id) return;
-                }
-                slot = (slot + 1 == nslots) ? 0u : slot + 1;
-                if (probes >= nslots) { atomicOr(&p.hdr->status, kStatusTableFull); return; }
-            }
-        };
-
+        // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list
         const uint32_t *ids = p.cand_ids + off0;
-        uint32_t head = (4u - (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u)) & 3u;
-        if (head > C) head = C;
-        const uint32_t nvec = (C - head) >> 2;
-        const uint32_t tail0 = head + (nvec << 2);
-        if (tid < head) insert(__ldg(ids + tid));
-        if (tid < C - tail0) insert(__ldg(ids + tail0 + tid));
-        const uint4 *v4 = reinterpret_cast<const uint4 *>(ids + head);
-        for (uint32_t v = tid; v < nvec; v += 2 * kDedupThreads) {
-            const uint4 x = __ldg(v4 + v);
-            const bool two = v + kDedupThreads < nvec;
-            uint4 y = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
-            if (two) y = __ldg(v4 + v + kDedupThreads);
-            insert(x.x); insert(x.y); insert(x.z); insert(x.w);
-            insert(y.x); insert(y.y); insert(y.z); insert(y.w);
-        }
+        const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
+        const uint32_t nvec = C ? (C + shift + 3u) >> 2 : 0u;
+        uint32_t v = tid;
+        const uint4 none4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+        uint4 nxt0 = none4, nxt1 = none4;                      // vectors v and v + kDedupThreads, in flight
+        if (v < nvec) nxt0 = load_ids4(ids, 4ll * v - shift, C);
+        if (v + kDedupThreads < nvec) nxt1 = load_ids4(ids, 4ll * (v + kDedupThreads) - shift, C);
+        uint32_t id[4] = {kIdNone, kIdNone, kIdNone, kIdNone}, slot[4] = {0, 0, 0, 0};
+        uint32_t stuck = 0;
+        for (;;) {
+            if ((id[0] & id[1] & id[2] & id[3]) == kIdNone && v < nvec) {      // nothing pending: next vector
+                id[0] = nxt0.x; id[1] = nxt0.y; id[2] = nxt0.z; id[3] = nxt0.w;
+                nxt0 = nxt1;
+                v += kDedupThreads;
+                if (v + kDedupThreads < nvec) nxt1 = load_ids4(ids, 4ll * (v + kDedupThreads) - shift, C);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) won += __shfl_xor_sync(0xffffffffu, won, o);
-        if (lane == 0 && won) atomicAdd(&misc[1], won);
+                for (int j = 0; j < 4; ++j) {
+                    const uint32_t x = id[j];
+                    uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
+                    const bool mine = x != kIdNone && (uint64_t)x < p.N && (S == 1 || __umulhi(a, S) == part);
+                    a = (a ^ (a >> 15)) * 0x846ca68bU;
+                    a ^= a >> 16;
+                    slot[j] = __umulhi(a, nslots);
+                    if (!mine) id[j] = kIdNone;
+                }
+                stuck = 0;
+            }
+            // read phase
+            bool put[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                put[j] = false;
+                if (id[j] != kIdNone) {
+                    const uint32_t cur = table[slot[j]];
+                    if (cur == id[j]) id[j] = kIdNone;
+                    else if (cur == kEmpty) put[j] = true;
+                    else slot[j] = slot[j] + 1 == nslots ? 0u : slot[j] + 1;
+                }
+            }
+            __syncthreads();
+            // write phase
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (put[j]) table[slot[j]] = id[j];
+            bool pending = (id[0] & id[1] & id[2] & id[3]) != kIdNone;
+            if (pending && ++stuck > 2 * nslots + 8) {             // table full (colliding IDs): give up on these
+                atomicOr(&p.hdr->status, kStatusTableFull);
+                id[0] = id[1] = id[2] = id[3] = kIdNone;
+                pending = false;
+            }
+            if (!__syncthreads_or(pending || v < nvec)) break;
+        }
+
+        // count the table, reserve the query's output range, compact into it
+        {
+            uint32_t c = 0;
+            for (uint32_t i = tid; i < nslots; i += kDedupThreads) c += table[i] != kEmpty ? 1u : 0u;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+            if (lane == 0 && c) atomicAdd(&misc[1], c);
+        }
         __syncthreads();
         if (tid == 0) misc[2] = atomicAdd(p.uniq_counts + b, misc[1]);
         __syncthreads();
-
-        // compact the table into the query's distinct list
         uint32_t *out = p.uniq_ids + off0 + misc[2];
         for (uint32_t base = tid - lane; base < nslots; base += kDedupThreads) {
             const uint32_t i = base + lane;
-            const uint32_t v = i < nslots ? table[i] : kEmpty;
-            const uint32_t bal = __ballot_sync(0xffffffffu, v != kEmpty);
+            const uint32_t v2 = i < nslots ? table[i] : kEmpty;
+            const uint32_t bal = __ballot_sync(0xffffffffu, v2 != kEmpty);
             if (bal) {
                 uint32_t pos = 0;
                 if (lane == 0) pos = atomicAdd(&misc[3], (uint32_t)__popc(bal));
                 pos = __shfl_sync(0xffffffffu, pos, 0);
-                if (v != kEmpty) out[pos + __popc(bal & lt_mask)] = v;
+                if (v2 != kEmpty) out[pos + __popc(bal & lt_mask)] = v2;
             }
         }
     }
@@ -567,17 +608,39 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 
 // ---------------------------------------------------------------- measurement: gather only
 
+// Load flavours the probe can compare (flavour 0 is what the scan kernel uses).
+__device__ __forceinline__ uint4 probe_load16(const void *p, uint32_t flavor, uint64_t pol)
+{
+    uint4 r;
+    switch (flavor) {
+    default: return ldg_nc_16(p);
+    case 1:
+        asm volatile("ld.global.nc.L1::no_allocate.L2::64B.v4.u32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+        return r;
+    case 2: return __ldg(reinterpret_cast<const uint4 *>(p));
+    case 3: return __ldcs(reinterpret_cast<const uint4 *>(p));
+    case 4:
+        asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                     : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p), "l"(pol));
+        return r;
+    case 5: return __ldcg(reinterpret_cast<const uint4 *>(p));
+    }
+}
+
 // Reads the code rows of ids[0 .. n) with the scan kernel's access pattern (G lanes per row, 16 bytes
 // each, NB*G loads in flight per lane) and xors them into sink: the row-gather ceiling of the scan.
 template <int G, int NB>
 __global__ void __launch_bounds__(kScanThreads) gather_probe_kernel(const uint8_t *__restrict__ codes,
                                                                     const uint32_t *__restrict__ ids, uint64_t n,
-                                                                    uint64_t N, uint32_t *sink)
+                                                                    uint64_t N, uint32_t *sink, uint32_t flavor)
 {
     constexpr int ROWB = 16 * G;
     const uint32_t lane = threadIdx.x & 31, q = lane & (G - 1);
     const uint64_t warp_global = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const uint64_t nwarps = ((uint64_t)gridDim.x * blockDim.x) >> 5;
+    uint64_t pol = 0;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     uint32_t acc = 0;
     for (uint64_t base = warp_global * 32 * NB; base < n; base += nwarps * 32 * NB) {
         uint32_t id[NB];
@@ -593,7 +656,7 @@ __global__ void __launch_bounds__(kScanThreads) gather_probe_kernel(const uint8_
 #pragma unroll
             for (int t = 0; t < G; ++t) {
                 const uint32_t rid = G == 1 ? id[nb] : __shfl_sync(0xffffffffu, id[nb], (lane & ~(G - 1)) | t);
-                rw[nb][t] = ldg_nc_16(codes + (uint64_t)rid * ROWB + q * 16);
+                rw[nb][t] = probe_load16(codes + (uint64_t)rid * ROWB + q * 16, flavor, pol);
             }
 #pragma unroll
         for (int nb = 0; nb < NB; ++nb)
@@ -601,6 +664,50 @@ __global__ void __launch_bounds__(kScanThreads) gather_probe_kernel(const uint8_
             for (int t = 0; t < G; ++t) acc ^= rw[nb][t].x ^ rw[nb][t].y ^ rw[nb][t].z ^ rw[nb][t].w;
     }
     if (acc == 0x9E3779B9u) sink[0] = acc;                      // keeps the loads alive; practically never true
+}
+
+// Same, with sm_100's 32-byte loads: H lanes per row (H = row_bytes / 32), 32 bytes each.
+template <int H, int NB>
+__global__ void __launch_bounds__(kScanThreads) gather_probe256_kernel(const uint8_t *__restrict__ codes,
+                                                                       const uint32_t *__restrict__ ids, uint64_t n,
+                                                                       uint64_t N, uint32_t *sink, uint32_t flavor)
+{
+    constexpr int ROWB = 32 * H;
+    const uint32_t lane = threadIdx.x & 31, q = lane & (H - 1);
+    const uint64_t warp_global = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const uint64_t nwarps = ((uint64_t)gridDim.x * blockDim.x) >> 5;
+    uint32_t acc = 0;
+    for (uint64_t base = warp_global * 32 * NB; base < n; base += nwarps * 32 * NB) {
+        uint32_t id[NB];
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb) {
+            const uint64_t idx = base + nb * 32 + lane;
+            id[nb] = idx < n ? __ldg(ids + idx) : 0u;
+            if ((uint64_t)id[nb] >= N) id[nb] = 0;
+        }
+        uint32_t rw[NB][H][8];
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb)
+#pragma unroll
+            for (int t = 0; t < H; ++t) {
+                const uint32_t rid = H == 1 ? id[nb] : __shfl_sync(0xffffffffu, id[nb], (lane & ~(H - 1)) | t);
+                const void *p = codes + (uint64_t)rid * ROWB + q * 32;
+                uint32_t *r = rw[nb][t];
+                if (flavor == 7)
+                    asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
+                else
+                    asm volatile("ld.global.nc.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
+            }
+#pragma unroll
+        for (int nb = 0; nb < NB; ++nb)
+#pragma unroll
+            for (int t = 0; t < H; ++t)
+#pragma unroll
+                for (int e = 0; e < 8; ++e) acc ^= rw[nb][t][e];
+    }
+    if (acc == 0x9E3779B9u) sink[0] = acc;
 }
 
 }  // namespace fann
