@@ -20,6 +20,7 @@ struct fann_index {
     int num_sms = 0;
     int smem_optin = 0;                    // max dynamic shared memory per block
     uint32_t chunks = 1;                   // batch chunks: dedup of chunk i+1 runs beside the scan of chunk i
+    uint32_t force_mode = 2;               // dedup placement: 0 ordered, 1 hashed, 2 decided per query (FANN_DEDUP_MODE)
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint64_t launches = 0;
     // second stream + events for the dedup/scan overlap
@@ -72,14 +73,14 @@ struct Geom {
 static void geometry(const fann_index *ix, uint32_t k, Geom *g)
 {
     g->dedup_smem = ix->dedup_smem;
-    g->nslots_max = ((g->dedup_smem - 64) / 4) & ~3u;
+    g->nslots_max = ((g->dedup_smem - 256) / 4) & ~3u;       // 256 bytes of CTA bookkeeping before the table
     g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
     g->cap = k <= 256 ? 4096u : 8192u;
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap);
 }
 
 struct WsLayout {
-    size_t hdr, S, item_start, items, uniq_counts, uniq_ids, total;
+    size_t hdr, S, mode, item_start, items, uniq_counts, uniq_ids, total;
     uint32_t max_items;
 };
 
@@ -90,6 +91,7 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
     size_t o = 0;
     w->hdr = o;         o = align_up(o + 256, 256);
     w->S = o;           o = align_up(o + (size_t)B * 4, 256);
+    w->mode = o;        o = align_up(o + (size_t)B * 4, 256);
     w->item_start = o;  o = align_up(o + ((size_t)B + 1) * 4, 256);
     w->items = o;       o = align_up(o + (size_t)w->max_items * 8, 256);
     w->uniq_counts = o; o = align_up(o + (size_t)B * 4, 256);
@@ -134,6 +136,7 @@ extern "C" int fann_create(fann_index **out, int device)
     ix->device = device; ix->num_sms = num_sms; ix->smem_optin = smem_optin;
     ix->dedup_smem = (uint32_t)smem_optin;
     if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
+    if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
     if (const char *s = getenv("FANN_L2_FETCH")) {
         int v = atoi(s);
         if (v == 32 || v == 64 || v == 128) CUDA_TRY(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)v));
@@ -328,6 +331,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     char *ws = (char *)workspace;
     WsHeader *hdr = (WsHeader *)(ws + w.hdr);
     uint32_t *S = (uint32_t *)(ws + w.S);
+    uint32_t *mode = (uint32_t *)(ws + w.mode);
     uint32_t *item_start = (uint32_t *)(ws + w.item_start);
     uint2 *items = (uint2 *)(ws + w.items);
     if (!dump) { uniq_counts = (uint32_t *)(ws + w.uniq_counts); uniq_ids = (uint32_t *)(ws + w.uniq_ids); }
@@ -336,8 +340,10 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     if (timing) cudaEventRecord(ix->ev_plan[0], stream);
     plan_kernel<<<1, 1024, 0, stream>>>((const long long *)cand_offsets, B, g.cap_c, w.max_items, hdr, S,
                                         item_start, items, uniq_counts);
+    mode_kernel<<<(B + 7) / 8, 256, 0, stream>>>((const long long *)cand_offsets, cand_ids, B, ix->N,
+                                                  ix->force_mode, mode);
     if (timing) cudaEventRecord(ix->ev_plan[1], stream);
-    ix->launches++;
+    ix->launches += 2;
     CUDA_TRY(cudaGetLastError());
 
     uint32_t chunks = dump ? 1u : ix->chunks;
@@ -351,7 +357,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
 
     DedupParams dp;
     dp.cand_offsets = (const long long *)cand_offsets; dp.cand_ids = cand_ids; dp.N = ix->N;
-    dp.nslots_max = g.nslots_max; dp.hdr = hdr; dp.S = S; dp.item_start = item_start; dp.items = items;
+    dp.nslots_max = g.nslots_max; dp.hdr = hdr; dp.S = S; dp.mode = mode; dp.item_start = item_start; dp.items = items;
     dp.uniq_ids = uniq_ids; dp.uniq_counts = uniq_counts;
     ScanParams sp;
     sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
@@ -523,11 +529,13 @@ extern "C" int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n
 {
     if (!ix || !ids || !sink) return fail(FANN_EINVAL, "fann_gather_probe: NULL argument");
     if (!ix->codes) return fail(FANN_EINVAL, "fann_gather_probe: load codes first");
+    const uint32_t mult = flavor >> 8;                  // bits 8..: CTAs per SM (0 = 2), for occupancy sweeps
+    flavor &= 0xffu;
     if (flavor > 7) return fail(FANN_EINVAL, "fann_gather_probe: flavor %u not in 0..7", flavor);
     if (flavor >= 6 && ix->row_bytes < 32) return fail(FANN_EUNSUPPORTED, "fann_gather_probe: 32-byte loads need rows >= 32 bytes");
     DeviceGuard guard(ix->device);
     cudaStream_t stream = (cudaStream_t)stream_;
-    const int grid = ix->num_sms * 2;
+    const int grid = ix->num_sms * (mult ? (int)mult : 2);
     if (flavor >= 6) {
         if (ix->row_bytes == 32) gather_probe256_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor);
         else gather_probe256_kernel<2, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor);

@@ -4,8 +4,10 @@
 //   repack_rows_kernel   fann_load_codes: pad rows of M bytes to 16 / 32 / 64 bytes
 //   build_lut_kernel     (1) lut[b][m][j] = sum_t (q - c)^2
 //   plan_kernel          split each query into S_b hash partitions that fit one SM's table
-//   dedup_kernel         (5) shared-memory hash dedup, one (query, partition) per CTA pass;
-//                        writes the distinct IDs of every query as a compact list
+//   mode_kernel          per query: order-preserving or hashed placement in the dedup table
+//   dedup_kernel         (5) shared-memory dedup table, one (query, partition) per CTA pass;
+//                        writes the distinct IDs of every query as a compact list, ascending
+//                        (up to probe displacement) in ordered mode
 //   scan_kernel          (6) code-row gather + Eq. 1 ADC  (7) streaming top-k, one query per
 //                        CTA pass; writes out_ids / out_dists / counts
 //   gather_probe_kernel  measurement only: the scan kernel's row gather without its arithmetic
@@ -173,6 +175,62 @@ __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t
 
 // ---------------------------------------------------------------- (5) dedup
 
+// Placement of the distinct IDs in the dedup table, per query:
+//   kModeOrdered  slot = floor((id - lo) * nslots / span): order-preserving, so the compacted table is
+//                 the distinct set in (almost) ascending ID order and the scan kernel's row gathers walk
+//                 the code array in address order (fewer address translations; measured 1.35-1.5x the
+//                 random-order gather rate).  Needs IDs that are spread evenly over [0, N).
+//   kModeHashed   slot = hash(id): for candidate lists whose IDs are bunched (runs of consecutive IDs,
+//                 one dense range), which would pile up in an order-preserving table.
+constexpr uint32_t kModeOrdered = 0, kModeHashed = 1;
+constexpr int kModeSamplePairs = 8;                  // adjacent pairs sampled per lane (256 per query)
+
+// One warp per query: sample 256 adjacent pairs of its candidate list and decide the placement mode.
+// Hashed if (a) some 1/32 range of [0, N) holds more than 3x its share of the samples, or (b) more than
+// 1/16 of the sampled neighbours are closer than N / (2 C) (about one table slot of the query).
+__global__ void mode_kernel(const long long *__restrict__ cand_offsets, const uint32_t *__restrict__ cand_ids,
+                            uint32_t B, uint64_t N, uint32_t force, uint32_t *__restrict__ mode)
+{
+    __shared__ uint32_t hist[8][32];
+    const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t b = blockIdx.x * 8 + w;
+    hist[w][lane] = 0;
+    __syncwarp();
+    if (b >= B) return;
+    const long long off0 = cand_offsets[b];
+    const long long Cll = cand_offsets[b + 1] - off0;
+    const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;
+    uint32_t m = kModeOrdered;
+    if (force < 2) {
+        m = force;
+    } else if (C >= 64 && N >= 64) {
+        const uint32_t *ids = cand_ids + off0;
+        const unsigned long long cd = N / (2ull * C);
+        const uint32_t close_dist = cd > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)cd;
+        const uint32_t ns = 32 * kModeSamplePairs;
+        const uint32_t bin_mul = (uint32_t)(((32ull << 32) - 1) / N);   // bin = id * 32 / N (< 32 for id < N)
+        uint32_t nvalid = 0, nclose = 0;
+#pragma unroll
+        for (int j = 0; j < kModeSamplePairs; ++j) {
+            const uint32_t i = j * 32 + lane;
+            const uint32_t e = (uint32_t)((unsigned long long)i * (C - 1) / ns);   // e + 1 <= C - 1
+            const uint32_t x = __ldg(ids + e), y = __ldg(ids + e + 1);
+            const bool vx = x != kIdNone && (uint64_t)x < N, vy = y != kIdNone && (uint64_t)y < N;
+            if (vx) { atomicAdd(&hist[w][__umulhi(x, bin_mul) & 31u], 1u); ++nvalid; }
+            if (vx && vy && x != y && (x > y ? x - y : y - x) < close_dist) ++nclose;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            nvalid += __shfl_xor_sync(0xffffffffu, nvalid, o);
+            nclose += __shfl_xor_sync(0xffffffffu, nclose, o);
+        }
+        __syncwarp();
+        const bool dense = hist[w][lane] > 3u * (nvalid / 32u) + 8u;
+        if (__any_sync(0xffffffffu, dense) || nclose * 16u > nvalid) m = kModeHashed;
+    }
+    if (lane == 0) mode[b] = m;
+}
+
 struct DedupParams {
     const long long *cand_offsets;                   // [B+1]
     const uint32_t *cand_ids;
@@ -182,6 +240,7 @@ struct DedupParams {
     uint32_t *counter;                               // work counter of this launch
     WsHeader *hdr;
     const uint32_t *S;                               // [B] partitions per query
+    const uint32_t *mode;                            // [B] kMode*
     const uint32_t *item_start;                      // [B+1]
     const uint2 *items;                              // [n_items] (query, partition)
     uint32_t *uniq_ids;                              // [total_cands]; query b's list starts at cand_offsets[b]
@@ -201,24 +260,29 @@ __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, ui
     return r;
 }
 
-// PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel
-// takes a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-
-// memory pipe on this part.  This kernel uses neither: open addressing with linear probing in shared
-// memory, advanced in CTA-wide rounds of a READ phase and a WRITE phase with a barrier after each.
-// Read phase: every pending ID reads its slot -- equal: done (a repeat, or its own store of the last
-// write phase survived); another ID: next slot; empty: store it in the write phase and look again.
-// No store is in flight during a read phase, so a slot seen non-empty keeps its value for good and
-// may be skipped safely; of several stores to one empty slot one survives and the losers see that in
-// the next read phase.  All copies of an ID walk the same probe sequence, so exactly one slot ends up
-// holding it.  Each CTA pass handles the IDs of one query that hash into one partition, then compacts
-// its table into the query's distinct list (order arbitrary).
+constexpr int kDedupIdsPerThread = 8;                // IDs a thread holds per batch (two 16-byte loads)
+
+// PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel takes
+// a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-memory
+// pipe on this part (64x a plain load).  This kernel uses neither: open addressing with linear probing
+// in shared memory, advanced in CTA-wide rounds with no store in flight while anyone reads:
+//   probe  (reads only)  every pending ID walks its probe sequence to its own value (a repeat: done)
+//                        or to the first empty slot;
+//   write                every still-pending ID stores itself into the empty slot it found;
+//   verify (reads only)  one of several stores to a slot survived; the losers (a few % of a batch) go
+//                        round again from that slot, which now holds another ID.
+// A slot seen non-empty keeps its value for good, all copies of an ID walk the same sequence, so exactly
+// one slot ends up holding it.  Each CTA pass handles the IDs of one query that fall into one partition
+// (an ID range in ordered mode, a hash class in hashed mode), 8 per thread per batch, then compacts its
+// table in slot order into the query's distinct list.
 __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupParams p)
 {
+    constexpr int R = kDedupIdsPerThread;
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] distinct here [2] out base [3] write pos
-    uint32_t *table = reinterpret_cast<uint32_t *>(smem + 64);
-    const uint32_t tid = threadIdx.x, lane = tid & 31;
-    const uint32_t lt_mask = (1u << lane) - 1u;
+    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base  [32..63] warp counts
+    uint32_t *wsum = misc + 32;
+    uint32_t *table = reinterpret_cast<uint32_t *>(smem + 256);
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t first = p.item_start[p.q_begin], last = p.item_start[p.q_end];
 
     for (;;) {
@@ -229,43 +293,58 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
         if (item >= last) break;
         const uint2 it = p.items[item];
         const uint32_t b = it.x, part = it.y, S = p.S[b];
+        const bool hashed = p.mode[b] == kModeHashed;
         const long long off0 = p.cand_offsets[b];
         const long long Cll = p.cand_offsets[b + 1] - off0;
         const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;       // plan guarantees C / S <= 0.75 nslots_max
 
-        // table sized to the partition: ~2.5 slots per candidate, never more than the CTA can hold
+        // table sized to the partition: 2 slots per candidate, never more than the CTA can hold
         uint32_t nslots = p.nslots_max;
         {
-            const unsigned long long want = ((unsigned long long)(C / S + 1) * 5 / 2 + 64) & ~3ull;
+            const unsigned long long want = ((unsigned long long)(C / S + 1) * 2 + 128) & ~3ull;
             if (want < nslots) nslots = (uint32_t)want;
+        }
+        // ordered mode: this partition owns IDs in [lo, lo + span); slot = (id - lo) * nslots / span
+        uint32_t lo = 0, span = 0, slot_mul = 0;
+        if (!hashed) {
+            const unsigned long long l = p.N * part / S, h = p.N * (part + 1ull) / S;
+            lo = (uint32_t)l; span = (uint32_t)(h - l);
+            slot_mul = span > nslots ? (uint32_t)(((unsigned long long)nslots << 32) / span) : 0u;   // 0: slot = id - lo
         }
         {
             uint4 *t4 = reinterpret_cast<uint4 *>(table);
             const uint4 e4 = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
             for (uint32_t i = tid; i < (nslots >> 2); i += kDedupThreads) t4[i] = e4;
-            if (tid == 0) { misc[1] = 0; misc[3] = 0; }
         }
-        __syncthreads();
 
         // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list
         const uint32_t *ids = p.cand_ids + off0;
         const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
         const uint32_t nvec = C ? (C + shift + 3u) >> 2 : 0u;
-        uint32_t v = tid;
         const uint4 none4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
-        uint4 nxt0 = none4, nxt1 = none4;                      // vectors v and v + kDedupThreads, in flight
-        if (v < nvec) nxt0 = load_ids4(ids, 4ll * v - shift, C);
-        if (v + kDedupThreads < nvec) nxt1 = load_ids4(ids, 4ll * (v + kDedupThreads) - shift, C);
-        uint32_t id[4] = {kIdNone, kIdNone, kIdNone, kIdNone}, slot[4] = {0, 0, 0, 0};
-        uint32_t stuck = 0;
-        for (;;) {
-            if ((id[0] & id[1] & id[2] & id[3]) == kIdNone && v < nvec) {      // nothing pending: next vector
-                id[0] = nxt0.x; id[1] = nxt0.y; id[2] = nxt0.z; id[3] = nxt0.w;
-                nxt0 = nxt1;
-                v += kDedupThreads;
-                if (v + kDedupThreads < nvec) nxt1 = load_ids4(ids, 4ll * (v + kDedupThreads) - shift, C);
+        uint4 nxt0 = none4, nxt1 = none4;                      // this thread's two vectors of the next batch
+        if (tid < nvec) nxt0 = load_ids4(ids, 4ll * tid - shift, C);
+        if (tid + kDedupThreads < nvec) nxt1 = load_ids4(ids, 4ll * (tid + kDedupThreads) - shift, C);
+        __syncthreads();                                       // table cleared
+
+        for (uint32_t vbase = 0; vbase < nvec; vbase += 2 * kDedupThreads) {
+            uint32_t id[R] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w};
+            uint32_t slot[R];
+            {
+                const uint32_t v = vbase + 2 * kDedupThreads + tid;
+                nxt0 = v < nvec ? load_ids4(ids, 4ll * v - shift, C) : none4;
+                nxt1 = v + kDedupThreads < nvec ? load_ids4(ids, 4ll * (v + kDedupThreads) - shift, C) : none4;
+            }
+            if (!hashed) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < R; ++j) {
+                    const uint32_t x = id[j] - lo;             // kIdNone and IDs >= N fall outside every span
+                    slot[j] = slot_mul ? __umulhi(x, slot_mul) : x;
+                    if (x >= span) id[j] = kIdNone;
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j];
                     uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
                     const bool mine = x != kIdNone && (uint64_t)x < p.N && (S == 1 || __umulhi(a, S) == part);
@@ -274,55 +353,87 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                     slot[j] = __umulhi(a, nslots);
                     if (!mine) id[j] = kIdNone;
                 }
-                stuck = 0;
             }
-            // read phase
-            bool put[4];
+            for (;;) {
+                // probe: to the ID itself (a repeat) or to the first empty slot
+                uint32_t cur[R];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                put[j] = false;
-                if (id[j] != kIdNone) {
-                    const uint32_t cur = table[slot[j]];
-                    if (cur == id[j]) id[j] = kIdNone;
-                    else if (cur == kEmpty) put[j] = true;
-                    else slot[j] = slot[j] + 1 == nslots ? 0u : slot[j] + 1;
+                for (int j = 0; j < R; ++j) cur[j] = id[j] != kIdNone ? table[slot[j]] : kEmpty;
+#pragma unroll
+                for (int j = 0; j < R; ++j) {
+                    if (id[j] == kIdNone) continue;
+                    uint32_t c = cur[j], s = slot[j], steps = 0;
+                    while (c != id[j] && c != kEmpty) {
+                        s = s + 1 == nslots ? 0u : s + 1;
+                        c = table[s];
+                        if (++steps > nslots) {                // table full of other IDs: give up on this one
+                            atomicOr(&p.hdr->status, kStatusTableFull);
+                            c = id[j];
+                        }
+                    }
+                    slot[j] = s;
+                    if (c == id[j]) id[j] = kIdNone;
                 }
-            }
-            __syncthreads();
-            // write phase
+                bool pending = false;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (put[j]) table[slot[j]] = id[j];
-            bool pending = (id[0] & id[1] & id[2] & id[3]) != kIdNone;
-            if (pending && ++stuck > 2 * nslots + 8) {             // table full (colliding IDs): give up on these
-                atomicOr(&p.hdr->status, kStatusTableFull);
-                id[0] = id[1] = id[2] = id[3] = kIdNone;
-                pending = false;
+                for (int j = 0; j < R; ++j) pending |= id[j] != kIdNone;
+                if (!__syncthreads_or(pending)) break;         // all reads done; nothing to store: batch done
+#pragma unroll
+                for (int j = 0; j < R; ++j)
+                    if (id[j] != kIdNone) table[slot[j]] = id[j];
+                __syncthreads();                               // all stores done
+#pragma unroll
+                for (int j = 0; j < R; ++j)
+                    if (id[j] != kIdNone && table[slot[j]] == id[j]) id[j] = kIdNone;
             }
-            if (!__syncthreads_or(pending || v < nvec)) break;
         }
 
-        // count the table, reserve the query's output range, compact into it
+        // compact the table in slot order: count per warp range, scan, write
         {
+            const uint4 *t4 = reinterpret_cast<const uint4 *>(table);
+            const uint32_t n4 = nslots >> 2;
+            const uint32_t chunk = ((n4 + kDedupThreads - 1) / kDedupThreads) * 32;   // vectors per warp, multiple of 32
+            const uint32_t v0 = warp * chunk < n4 ? warp * chunk : n4;
+            const uint32_t v1 = v0 + chunk < n4 ? v0 + chunk : n4;
             uint32_t c = 0;
-            for (uint32_t i = tid; i < nslots; i += kDedupThreads) c += table[i] != kEmpty ? 1u : 0u;
+            for (uint32_t v = v0 + lane; v < v1; v += 32) {
+                const uint4 t = t4[v];
+                c += (t.x != kEmpty) + (t.y != kEmpty) + (t.z != kEmpty) + (t.w != kEmpty);
+            }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-            if (lane == 0 && c) atomicAdd(&misc[1], c);
-        }
-        __syncthreads();
-        if (tid == 0) misc[2] = atomicAdd(p.uniq_counts + b, misc[1]);
-        __syncthreads();
-        uint32_t *out = p.uniq_ids + off0 + misc[2];
-        for (uint32_t base = tid - lane; base < nslots; base += kDedupThreads) {
-            const uint32_t i = base + lane;
-            const uint32_t v2 = i < nslots ? table[i] : kEmpty;
-            const uint32_t bal = __ballot_sync(0xffffffffu, v2 != kEmpty);
-            if (bal) {
-                uint32_t pos = 0;
-                if (lane == 0) pos = atomicAdd(&misc[3], (uint32_t)__popc(bal));
-                pos = __shfl_sync(0xffffffffu, pos, 0);
-                if (v2 != kEmpty) out[pos + __popc(bal & lt_mask)] = v2;
+            if (lane == 0) wsum[warp] = c;
+            __syncthreads();
+            if (warp == 0) {
+                const uint32_t wv = wsum[lane];
+                uint32_t incl = wv;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += u;
+                }
+                wsum[lane] = incl - wv;                        // exclusive
+                if (lane == 31) misc[1] = incl ? atomicAdd(p.uniq_counts + b, incl) : 0u;
+            }
+            __syncthreads();
+            uint32_t *out = p.uniq_ids + off0 + misc[1];
+            uint32_t run = wsum[warp];
+            for (uint32_t vb = v0; vb < v1; vb += 32) {
+                const uint32_t v = vb + lane;
+                const uint4 t = v < v1 ? t4[v] : make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
+                const uint32_t cnt = (t.x != kEmpty) + (t.y != kEmpty) + (t.z != kEmpty) + (t.w != kEmpty);
+                uint32_t incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += u;
+                }
+                uint32_t pos = run + incl - cnt;
+                if (t.x != kEmpty) out[pos++] = t.x;
+                if (t.y != kEmpty) out[pos++] = t.y;
+                if (t.z != kEmpty) out[pos++] = t.z;
+                if (t.w != kEmpty) out[pos++] = t.w;
+                run += __shfl_sync(0xffffffffu, incl, 31);
             }
         }
     }

@@ -132,7 +132,9 @@ def test_lut_query_on_centroid_is_exact_zero(fann, tiny):
 
 # ------------------------------------------------------------------ (5) dedup
 
-def _dedup_check(fann, w, off, ids):
+def _dedup_check(fann, w, off, ids, ascending=None):
+    """ascending: query indices whose distinct list must come out non-decreasing (one partition,
+    ordered placement) except for the few IDs displaced by probing."""
     ix = fann.FannIndex(0)
     ix.load_codes(w.codes.to(DEV))
     o = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int64)).to(DEV)
@@ -145,6 +147,9 @@ def _dedup_check(fann, w, off, ids):
         got = uids[off[b]:off[b] + ucnt[b]]
         assert ucnt[b] == want.size, f"query {b}: {ucnt[b]} != {want.size}"
         assert np.array_equal(np.sort(got), want), f"query {b}: distinct sets differ"
+        if ascending and b in ascending and got.size > 1:
+            inversions = np.count_nonzero(np.diff(got.astype(np.int64)) < 0)
+            assert inversions <= 0.25 * got.size, f"query {b}: {inversions} descents in {got.size} ids"
 
 
 def test_dedup_sets_bit_exact(fann, tiny_local, w_int, w_k1000):
@@ -168,6 +173,31 @@ def test_dedup_adversarial(fann, tiny_local):
     off = np.zeros(len(lists) + 1, dtype=np.int64)
     off[1:] = np.cumsum([len(x) for x in lists])
     _dedup_check(fann, w, off, np.concatenate(lists))
+
+
+def _bunched_lists(N, rng):
+    """Candidate lists whose IDs are NOT spread evenly over [0, N): the order-preserving table
+    would pile them up, so the library must fall back to hashed placement."""
+    runs = np.concatenate([np.arange(s, s + 400, dtype=np.uint32) for s in rng.integers(0, N - 400, size=60)])
+    dense = rng.integers(N // 3, N // 3 + 30_000, size=45_000).astype(np.uint32)         # one narrow range
+    half = np.concatenate([rng.integers(0, N // 64, size=20_000), rng.integers(0, N, size=5_000)]).astype(np.uint32)
+    spread = rng.permutation(N)[:30_000].astype(np.uint32)                               # evenly spread: ordered
+    return [np.concatenate([runs, runs[::-1]]), dense, rng.permutation(half), spread]
+
+
+@pytest.mark.parametrize("force", [None, "0", "1"])
+def test_dedup_placement_modes(fann, tiny_local, monkeypatch, force):
+    """Ordered, hashed and per-query placement give the same distinct sets; evenly spread lists come
+    out ascending when the placement is ordered (what the scan kernel's gather relies on for speed)."""
+    if force is None:
+        monkeypatch.delenv("FANN_DEDUP_MODE", raising=False)
+    else:
+        monkeypatch.setenv("FANN_DEDUP_MODE", force)
+    w = tiny_local
+    lists = _bunched_lists(w.cfg.N, np.random.default_rng(11))
+    off = np.zeros(len(lists) + 1, dtype=np.int64)
+    off[1:] = np.cumsum([len(x) for x in lists])
+    _dedup_check(fann, w, off, np.concatenate(lists), ascending=None if force == "1" else {3})
 
 
 # ------------------------------------------------------------------ whole path
