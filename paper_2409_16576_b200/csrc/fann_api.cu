@@ -73,7 +73,7 @@ struct Geom {
 static void geometry(const fann_index *ix, uint32_t k, Geom *g)
 {
     g->dedup_smem = ix->dedup_smem;
-    g->nslots_max = ((g->dedup_smem - 256) / 4) & ~3u;       // 256 bytes of CTA bookkeeping before the table
+    g->nslots_max = ((g->dedup_smem - kDedupTableOff) / 4) & ~3u;
     g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
     g->cap = k <= 256 ? 4096u : 8192u;
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap);

@@ -261,6 +261,7 @@ __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, ui
 }
 
 constexpr int kDedupIdsPerThread = 8;                // IDs a thread holds per batch (two 16-byte loads)
+constexpr uint32_t kDedupTableOff = 256 + 2 * kDedupThreads * 4;   // bookkeeping + two retry queues precede the table
 
 // PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel takes
 // a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-memory
@@ -269,8 +270,8 @@ constexpr int kDedupIdsPerThread = 8;                // IDs a thread holds per b
 //   probe  (reads only)  every pending ID walks its probe sequence to its own value (a repeat: done)
 //                        or to the first empty slot;
 //   write                every still-pending ID stores itself into the empty slot it found;
-//   verify (reads only)  one of several stores to a slot survived; the losers (a few % of a batch) go
-//                        round again from that slot, which now holds another ID.
+//   verify (reads only)  one of several stores to a slot survived; the losers (a few per batch) enter a
+//                        small queue and are taken up again, one per thread, with the next batch.
 // A slot seen non-empty keeps its value for good, all copies of an ID walk the same sequence, so exactly
 // one slot ends up holding it.  Each CTA pass handles the IDs of one query that fall into one partition
 // (an ID range in ordered mode, a hash class in hashed mode), 8 per thread per batch, then compacts its
@@ -279,9 +280,10 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 {
     constexpr int R = kDedupIdsPerThread;
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base  [32..63] warp counts
-    uint32_t *wsum = misc + 32;
-    uint32_t *table = reinterpret_cast<uint32_t *>(smem + 256);
+    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base [2,3] queue lengths [32..63] warp counts
+    uint32_t *wsum = misc + 32, *qcnt = misc + 2;
+    uint32_t *queue = reinterpret_cast<uint32_t *>(smem + 256);              // two retry queues of kDedupThreads IDs
+    uint32_t *table = reinterpret_cast<uint32_t *>(smem + kDedupTableOff);
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t first = p.item_start[p.q_begin], last = p.item_start[p.q_end];
 
@@ -317,24 +319,39 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
             for (uint32_t i = tid; i < (nslots >> 2); i += kDedupThreads) t4[i] = e4;
         }
 
-        // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list
+        // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list.
+        // Vectors [v_in0, v_in1) lie wholly inside the list and are read with one 16-byte load.
         const uint32_t *ids = p.cand_ids + off0;
         const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
+        const uint4 *ids4 = reinterpret_cast<const uint4 *>(ids - shift);
         const uint32_t nvec = C ? (C + shift + 3u) >> 2 : 0u;
+        const uint32_t v_in0 = shift ? 1u : 0u, v_in1 = (C + shift) >> 2;
         const uint4 none4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
-        uint4 nxt0 = none4, nxt1 = none4;                      // this thread's two vectors of the next batch
-        if (tid < nvec) nxt0 = load_ids4(ids, 4ll * tid - shift, C);
-        if (tid + kDedupThreads < nvec) nxt1 = load_ids4(ids, 4ll * (tid + kDedupThreads) - shift, C);
-        __syncthreads();                                       // table cleared
+        auto load_vec = [&](uint32_t v) -> uint4 {
+            if (v >= v_in0 && v < v_in1) return __ldg(ids4 + v);
+            if (v < nvec) return load_ids4(ids, 4ll * v - shift, C);
+            return none4;
+        };
+        // slot of a valid ID of this partition
+        auto place = [&](uint32_t x) -> uint32_t {
+            if (!hashed) return slot_mul ? __umulhi(x - lo, slot_mul) : x - lo;
+            uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
+            a = (a ^ (a >> 15)) * 0x846ca68bU;
+            a ^= a >> 16;
+            return __umulhi(a, nslots);
+        };
+        uint4 nxt0 = load_vec(tid), nxt1 = load_vec(tid + kDedupThreads);   // this thread's vectors of the next batch
+        if (tid == 0) { qcnt[0] = 0; qcnt[1] = 0; }
+        __syncthreads();                                       // table cleared, queues empty
 
-        for (uint32_t vbase = 0; vbase < nvec; vbase += 2 * kDedupThreads) {
-            uint32_t id[R] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w};
-            uint32_t slot[R];
-            {
-                const uint32_t v = vbase + 2 * kDedupThreads + tid;
-                nxt0 = v < nvec ? load_ids4(ids, 4ll * v - shift, C) : none4;
-                nxt1 = v + kDedupThreads < nvec ? load_ids4(ids, 4ll * (v + kDedupThreads) - shift, C) : none4;
-            }
+        // Batches of 8 fresh IDs per thread plus one ID from the retry queue (IDs that lost a store race
+        // in the batch before).  After the list is exhausted the loop runs on until the queue is empty.
+        uint32_t qin = 0, qn = 0;                              // queue read by this batch, its length
+        for (uint32_t vbase = 0; vbase < nvec || qn; vbase += 2 * kDedupThreads) {
+            uint32_t id[R + 1] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w, kIdNone};
+            uint32_t slot[R + 1];
+            nxt0 = load_vec(vbase + 2 * kDedupThreads + tid);
+            nxt1 = load_vec(vbase + 3 * kDedupThreads + tid);
             if (!hashed) {
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
@@ -346,46 +363,79 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j];
-                    uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
+                    const uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
                     const bool mine = x != kIdNone && (uint64_t)x < p.N && (S == 1 || __umulhi(a, S) == part);
-                    a = (a ^ (a >> 15)) * 0x846ca68bU;
-                    a ^= a >> 16;
-                    slot[j] = __umulhi(a, nslots);
+                    slot[j] = place(x);
                     if (!mine) id[j] = kIdNone;
                 }
             }
+            slot[R] = 0;
+            if (tid < qn) { id[R] = queue[qin * kDedupThreads + tid]; slot[R] = place(id[R]); }
+            uint32_t *qpush = queue + (qin ^ 1u) * kDedupThreads;
             for (;;) {
-                // probe: to the ID itself (a repeat) or to the first empty slot
-                uint32_t cur[R];
+                // probe (reads only): to the ID itself (a repeat) or to the first empty slot.
+                // kIdNone == kEmpty, so an absent ID "finds itself" and needs no special case.
+                uint32_t cur[R + 1];
 #pragma unroll
-                for (int j = 0; j < R; ++j) cur[j] = id[j] != kIdNone ? table[slot[j]] : kEmpty;
+                for (int j = 0; j <= R; ++j) cur[j] = id[j] != kIdNone ? table[slot[j]] : kEmpty;
+                uint32_t unres = 0;
 #pragma unroll
-                for (int j = 0; j < R; ++j) {
-                    if (id[j] == kIdNone) continue;
-                    uint32_t c = cur[j], s = slot[j], steps = 0;
-                    while (c != id[j] && c != kEmpty) {
-                        s = s + 1 == nslots ? 0u : s + 1;
-                        c = table[s];
-                        if (++steps > nslots) {                // table full of other IDs: give up on this one
-                            atomicOr(&p.hdr->status, kStatusTableFull);
-                            c = id[j];
-                        }
-                    }
-                    slot[j] = s;
-                    if (c == id[j]) id[j] = kIdNone;
+                for (int j = 0; j <= R; ++j) {
+                    if (cur[j] != id[j] && cur[j] != kEmpty) unres |= 1u << j;
+                    if (cur[j] == id[j]) id[j] = kIdNone;
                 }
-                bool pending = false;
+                if (unres) {                                   // occupied by another ID: walk on
 #pragma unroll
-                for (int j = 0; j < R; ++j) pending |= id[j] != kIdNone;
-                if (!__syncthreads_or(pending)) break;         // all reads done; nothing to store: batch done
+                    for (int j = 0; j <= R; ++j) {
+                        if (!(unres & (1u << j))) continue;
+                        uint32_t c, s = slot[j], steps = 0;
+                        do {
+                            s = s + 1 == nslots ? 0u : s + 1;
+                            c = table[s];
+                            if (++steps > nslots) {            // table full of other IDs: give up on this one
+                                atomicOr(&p.hdr->status, kStatusTableFull);
+                                c = id[j];
+                            }
+                        } while (c != id[j] && c != kEmpty);
+                        slot[j] = s;
+                        if (c == id[j]) id[j] = kIdNone;
+                    }
+                }
+                uint32_t all = id[0];
 #pragma unroll
-                for (int j = 0; j < R; ++j)
+                for (int j = 1; j <= R; ++j) all &= id[j];
+                const bool any_store = __syncthreads_or(all != kIdNone);   // all reads done
+                if (tid == 0) qcnt[qin] = 0;                   // drained queue: its length was read before this barrier
+                if (!any_store) break;                         // nothing to store: batch done
+#pragma unroll
+                for (int j = 0; j <= R; ++j)
                     if (id[j] != kIdNone) table[slot[j]] = id[j];
                 __syncthreads();                               // all stores done
+                // verify (reads only): of several stores to one slot one survived
 #pragma unroll
-                for (int j = 0; j < R; ++j)
-                    if (id[j] != kIdNone && table[slot[j]] == id[j]) id[j] = kIdNone;
+                for (int j = 0; j <= R; ++j) cur[j] = id[j] != kIdNone ? table[slot[j]] : kEmpty;
+                all = kIdNone;
+#pragma unroll
+                for (int j = 0; j <= R; ++j) {
+                    if (cur[j] == id[j]) id[j] = kIdNone;
+                    all &= id[j];
+                }
+                if (all != kIdNone) {                          // losers: retry with the next batch
+#pragma unroll
+                    for (int j = 0; j <= R; ++j) {
+                        if (id[j] == kIdNone) continue;
+                        const uint32_t pos = atomicAdd(&qcnt[qin ^ 1u], 1u);
+                        if (pos < (uint32_t)kDedupThreads) { qpush[pos] = id[j]; id[j] = kIdNone; }
+                    }
+                    all = id[0];
+#pragma unroll
+                    for (int j = 1; j <= R; ++j) all &= id[j];
+                }
+                if (!__syncthreads_or(all != kIdNone)) break;  // queue full (IDs chosen to collide): go round again
             }
+            qin ^= 1u;                                         // the queue just filled is the next batch's input
+            qn = qcnt[qin];
+            if (qn > (uint32_t)kDedupThreads) qn = kDedupThreads;
         }
 
         // compact the table in slot order: count per warp range, scan, write
