@@ -41,7 +41,7 @@ struct WsHeader {                                    // first 256 bytes of the w
 __device__ __forceinline__ uint4 ldg_nc_16(const void *p)
 {
     uint4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+    asm volatile("ld.global.nc.L1::no_allocate.L2::64B.v4.u32 {%0,%1,%2,%3}, [%4];"   // default fetches 128 B from DRAM
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
     return r;
 }
@@ -542,7 +542,7 @@ __device__ __forceinline__ void prune(unsigned long long *buf, uint32_t *misc, u
     const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t n = vm[0];
     if (tid < kSample) { samp[tid] = buf[(unsigned long long)tid * n / kSample]; rank[tid] = 0; }
-    if (tid == 0) *pivot_p = kKeyMax - 1;
+    if (tid == 0) { *pivot_p = kKeyMax - 1; misc[9] = 0; }
     __syncthreads();
     {
         constexpr int parts = kScanThreads / kSample, len = kSample / parts;
@@ -669,7 +669,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
         const uint32_t beta = (uint32_t)j ^ x0;
         sel[j] = (4u + beta) | (beta << 4) | ((8u | (4u + beta)) << 8) | ((8u | (4u + beta)) << 12);
     }
-    const uint32_t margin = kScanWarps * 32 * NB;              // keys one CTA iteration can append
+    const uint32_t margin = kScanWarps * 32 * NB + 64;         // keys appended between the buffer passing its limit and the prune
     const uint32_t limit = p.cap - margin;
 
     for (;;) {
@@ -693,14 +693,22 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                 float *d = luts + (c4 * 4) * 64 + col;
                 d[0] = v.x; d[64] = v.y; d[128] = v.z; d[192] = v.w;
             }
-            if (tid == 0) { misc[0] = 0; *tau_p = kKeyMax; }
+            if (tid == 0) { misc[0] = 0; misc[9] = 0; *tau_p = kKeyMax; }
         }
         __syncthreads();
 
         const uint32_t per_iter = kScanWarps * 32 * NB;
         const uint32_t n_iter = (U + per_iter - 1) / per_iter;
-        for (uint32_t itn = 0; itn < n_iter; ++itn) {
+        // Warps run free: no barrier per iteration.  The warp whose append takes the buffer past its limit
+        // raises misc[9]; every warp sees it before its next iteration (each appends at most one more
+        // iteration's keys, which the margin above the limit holds) and meets the others at the barrier
+        // below, where the buffer is pruned.  A warp out of work waits there too, so the barrier completes
+        // exactly when every warp is done or has seen the flag.
+        uint32_t itn = 0;
+        for (;;) {
+          while (itn < n_iter && !vm[9]) {
             const uint32_t base = (itn * kScanWarps + warp) * 32 * NB;
+            ++itn;
             if (base < U) {
                 uint32_t id[NB];
 #pragma unroll
@@ -738,8 +746,11 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                         if (keep) buf[pos + __popc(bal & lt_mask)] = key;
                     }
                 }
+                if (lane == 0 && vm[0] > limit) vm[9] = 1;
             }
-            if (__syncthreads_or(vm[0] > limit)) prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
+          }
+          if (!__syncthreads_or(vm[9] != 0)) break;
+          prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
         }
 
         // exact top-k of what is left
