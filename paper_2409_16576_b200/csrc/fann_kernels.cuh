@@ -46,6 +46,18 @@ __device__ __forceinline__ uint4 ldg_nc_16(const void *p)
     return r;
 }
 
+// Shared-memory access by 32-bit shared-window address (no generic-address arithmetic per access).
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.u32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
+}
+
 // Block-wide bitonic sort (ascending) of n = 2^p keys in shared memory,
 // starting from sorted runs of length first_size / 2.
 __device__ __forceinline__ void bitonic_sort_smem(unsigned long long *a, uint32_t n, uint32_t first_size)
@@ -280,12 +292,15 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 {
     constexpr int R = kDedupIdsPerThread;
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base [2,3] queue lengths [32..63] warp counts
+    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base [2,3] queue lengths [4] kEmpty [32..63] warp counts
     uint32_t *wsum = misc + 32, *qcnt = misc + 2;
     uint32_t *queue = reinterpret_cast<uint32_t *>(smem + 256);              // two retry queues of kDedupThreads IDs
     uint32_t *table = reinterpret_cast<uint32_t *>(smem + kDedupTableOff);
+    const uint32_t tbl = (uint32_t)__cvta_generic_to_shared(table);
+    const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 4);   // a word that always holds kEmpty
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t first = p.item_start[p.q_begin], last = p.item_start[p.q_end];
+    if (tid == 0) misc[4] = kEmpty;
 
     for (;;) {
         __syncthreads();                                       // previous item fully done
@@ -332,32 +347,38 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
             if (v < nvec) return load_ids4(ids, 4ll * v - shift, C);
             return none4;
         };
-        // slot of a valid ID of this partition
+        // shared-memory byte address of the home slot of a valid ID of this partition
         auto place = [&](uint32_t x) -> uint32_t {
-            if (!hashed) return slot_mul ? __umulhi(x - lo, slot_mul) : x - lo;
+            if (!hashed) return tbl + ((slot_mul ? __umulhi(x - lo, slot_mul) : x - lo) << 2);
             uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
             a = (a ^ (a >> 15)) * 0x846ca68bU;
             a ^= a >> 16;
-            return __umulhi(a, nslots);
+            return tbl + (__umulhi(a, nslots) << 2);
         };
+        const uint32_t tbl_end = tbl + (nslots << 2);
         uint4 nxt0 = load_vec(tid), nxt1 = load_vec(tid + kDedupThreads);   // this thread's vectors of the next batch
         if (tid == 0) { qcnt[0] = 0; qcnt[1] = 0; }
         __syncthreads();                                       // table cleared, queues empty
 
         // Batches of 8 fresh IDs per thread plus one ID from the retry queue (IDs that lost a store race
         // in the batch before).  After the list is exhausted the loop runs on until the queue is empty.
+        // sa[j] is the shared-memory byte address of the slot ID j looks at.  An absent ID (kIdNone) looks
+        // at `none_addr`, a word that always holds kEmpty == kIdNone: it "finds itself" there, so probe and
+        // verify need no special case and no predicated loads.
         uint32_t qin = 0, qn = 0;                              // queue read by this batch, its length
         for (uint32_t vbase = 0; vbase < nvec || qn; vbase += 2 * kDedupThreads) {
             uint32_t id[R + 1] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w, kIdNone};
-            uint32_t slot[R + 1];
+            uint32_t sa[R + 1];
             nxt0 = load_vec(vbase + 2 * kDedupThreads + tid);
             nxt1 = load_vec(vbase + 3 * kDedupThreads + tid);
             if (!hashed) {
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j] - lo;             // kIdNone and IDs >= N fall outside every span
-                    slot[j] = slot_mul ? __umulhi(x, slot_mul) : x;
-                    if (x >= span) id[j] = kIdNone;
+                    const uint32_t a = tbl + ((slot_mul ? __umulhi(x, slot_mul) : x) << 2);
+                    const bool mine = x < span;
+                    sa[j] = mine ? a : none_addr;
+                    if (!mine) id[j] = kIdNone;
                 }
             } else {
 #pragma unroll
@@ -365,40 +386,40 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                     const uint32_t x = id[j];
                     const uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
                     const bool mine = x != kIdNone && (uint64_t)x < p.N && (S == 1 || __umulhi(a, S) == part);
-                    slot[j] = place(x);
+                    sa[j] = mine ? place(x) : none_addr;
                     if (!mine) id[j] = kIdNone;
                 }
             }
-            slot[R] = 0;
-            if (tid < qn) { id[R] = queue[qin * kDedupThreads + tid]; slot[R] = place(id[R]); }
+            sa[R] = none_addr;
+            if (tid < qn) { id[R] = queue[qin * kDedupThreads + tid]; sa[R] = place(id[R]); }
             uint32_t *qpush = queue + (qin ^ 1u) * kDedupThreads;
             for (;;) {
-                // probe (reads only): to the ID itself (a repeat) or to the first empty slot.
-                // kIdNone == kEmpty, so an absent ID "finds itself" and needs no special case.
+                // probe (reads only): to the ID itself (a repeat) or to the first empty slot
                 uint32_t cur[R + 1];
 #pragma unroll
-                for (int j = 0; j <= R; ++j) cur[j] = id[j] != kIdNone ? table[slot[j]] : kEmpty;
-                uint32_t unres = 0;
+                for (int j = 0; j <= R; ++j) cur[j] = lds_u32(sa[j]);
+                bool unres = false;
 #pragma unroll
                 for (int j = 0; j <= R; ++j) {
-                    if (cur[j] != id[j] && cur[j] != kEmpty) unres |= 1u << j;
+                    unres |= cur[j] != id[j] && cur[j] != kEmpty;
                     if (cur[j] == id[j]) id[j] = kIdNone;
                 }
-                if (unres) {                                   // occupied by another ID: walk on
+                if (unres) {                                   // some slot held another ID: walk on
 #pragma unroll
                     for (int j = 0; j <= R; ++j) {
-                        if (!(unres & (1u << j))) continue;
-                        uint32_t c, s = slot[j], steps = 0;
+                        if (cur[j] == kEmpty || id[j] == kIdNone) continue;
+                        uint32_t c, a = sa[j], steps = 0;
                         do {
-                            s = s + 1 == nslots ? 0u : s + 1;
-                            c = table[s];
+                            a += 4;
+                            if (a == tbl_end) a = tbl;
+                            c = lds_u32(a);
                             if (++steps > nslots) {            // table full of other IDs: give up on this one
                                 atomicOr(&p.hdr->status, kStatusTableFull);
                                 c = id[j];
                             }
                         } while (c != id[j] && c != kEmpty);
-                        slot[j] = s;
-                        if (c == id[j]) id[j] = kIdNone;
+                        sa[j] = a;
+                        if (c == id[j]) { id[j] = kIdNone; sa[j] = none_addr; }
                     }
                 }
                 uint32_t all = id[0];
@@ -409,11 +430,11 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                 if (!any_store) break;                         // nothing to store: batch done
 #pragma unroll
                 for (int j = 0; j <= R; ++j)
-                    if (id[j] != kIdNone) table[slot[j]] = id[j];
+                    if (id[j] != kIdNone) sts_u32(sa[j], id[j]);
                 __syncthreads();                               // all stores done
                 // verify (reads only): of several stores to one slot one survived
 #pragma unroll
-                for (int j = 0; j <= R; ++j) cur[j] = id[j] != kIdNone ? table[slot[j]] : kEmpty;
+                for (int j = 0; j <= R; ++j) cur[j] = lds_u32(sa[j]);
                 all = kIdNone;
 #pragma unroll
                 for (int j = 0; j <= R; ++j) {
@@ -425,7 +446,7 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                     for (int j = 0; j <= R; ++j) {
                         if (id[j] == kIdNone) continue;
                         const uint32_t pos = atomicAdd(&qcnt[qin ^ 1u], 1u);
-                        if (pos < (uint32_t)kDedupThreads) { qpush[pos] = id[j]; id[j] = kIdNone; }
+                        if (pos < (uint32_t)kDedupThreads) { qpush[pos] = id[j]; id[j] = kIdNone; sa[j] = none_addr; }
                     }
                     all = id[0];
 #pragma unroll
