@@ -224,11 +224,16 @@ def main():
 
     # ---- roofline of the dominant kernel (scan: dedup + gather + ADC + local top-k)
     peak, peak_src = measured_peak_gbs()
-    algo_bytes = M * U_total + 4 * total + 1024 * M * B + 8 * k * B
+    # scan kernel's own algorithmic bytes: code rows + distinct IDs + tables + outputs
+    algo_bytes = M * U_total + 4 * U_total + 1024 * M * B + 8 * k * B
+    path_bytes = algo_bytes + 4 * total + 4 * U_total                          # + dedup: IDs read, distinct IDs written
     scan_ms = float(np.mean(kern["scan_ms"]))
     achieved = algo_bytes / (scan_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "scan_kernel", "achieved": round(achieved, 1), "peak": peak,
-                "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": None,
+                "unit": "GB/s", "frac": round(achieved / peak, 4),
+                # dram__bytes_read+write per gathered row from the committed ncu --set full capture of this kernel
+                # (profiles/r1e_scan_kernel_rows64_ncu.txt, 64-byte rows), scaled to this launch; null for other rows
+                "traffic": int(68.5 * U_total) if M > 32 else None,
                 "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kernel_ms": round(scan_ms, 4),
                 "code_bytes_only_frac": round(M * U_total / (scan_ms * 1e-3) / 1e9 / peak, 4),
                 "share_of_step": round(scan_ms / ms_per_step, 4),
@@ -294,6 +299,7 @@ def main():
                "batch_qps": nq / dt, "gpu_matches_oracle_on_sample": parity}
 
     line = {
+        "path_algorithmic_bytes": path_bytes, "path_hbm_frac": round(path_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4),
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
