@@ -107,6 +107,25 @@ def oracle_sample(w, n_queries: int, codes_dev, nthreads: int = 0):
     return dt, r, int(r["uniq"].sum())
 
 
+def aggregate_over_ranks(total_ms: float, units: float, inputs: float, device=None):
+    """Replicas only: the job's time is the MAX over ranks, its work the SUM.  Uses the
+    default process group if one is initialised (nccl on GPUs; gloo in the CPU test), else passes through."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(total_ms), float(units), float(inputs)
+    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([units, inputs], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u[0].item()), float(u[1].item())
+
+
+def rank_seed(base_seed: int, rank: int) -> int:
+    """Every replica scores its own batch: rank r draws its workload from seed base + r."""
+    return base_seed + rank
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -149,7 +168,7 @@ def main():
     build()
 
     t_gen = time.time()
-    w = make_workload(cfg, seed=DEFAULT_SEED + rank, device=dev)     # each replica: its own batch
+    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev)     # each replica: its own batch
     torch.cuda.synchronize()
     t_gen = time.time() - t_gen
     B, k, M, dsub = cfg.B, cfg.k, cfg.M, cfg.dsub
@@ -209,16 +228,7 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
     clocks = sampler.stop(t0, t1) if sampler else None
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-        u = torch.tensor([U_total, total], device=dev, dtype=torch.float64)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        U_all, C_all = float(u[0].item()), float(u[1].item())
-    else:
-        U_all, C_all = float(U_total), float(total)
+    total_ms, U_all, C_all = aggregate_over_ranks(total_ms, U_total, total, device=dev)
     ms_per_step = total_ms / args.steps
     value = U_all / (ms_per_step * 1e-3)
 

@@ -209,6 +209,8 @@ int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup
  * in flight and threads per CTA) and do nothing else.  Timed by the caller, it
  * gives the rate at which this GPU can gather those rows at all -- the practical
  * ceiling of step (6).  IDs >= N read row 0.
+ * flavor bits 0-7: load instruction (0 plain 16-byte non-coherent loads, 1 the scan kernel's: the same with a 64-byte
+ * L2 fetch, 2-5 other cache hints, 6-7 32-byte loads); bits 8 and up: CTAs per SM (0 = 2).
  * ids  device, [n] uint32      sink  device, 4 bytes (never written in practice)
  */
 int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink,
