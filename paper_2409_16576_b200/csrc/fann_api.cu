@@ -21,6 +21,7 @@ struct fann_index {
     int smem_optin = 0;                    // max dynamic shared memory per block
     uint32_t chunks = 1;                   // batch chunks: dedup of chunk i+1 runs beside the scan of chunk i
     uint32_t force_mode = 2;               // dedup placement: 0 ordered, 1 hashed, 2 decided per query (FANN_DEDUP_MODE)
+    bool partition = true;                 // split lists into their dedup classes first (FANN_PARTITION=0: filter per pass)
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint64_t launches = 0;
     // second stream + events for the dedup/scan overlap
@@ -80,7 +81,7 @@ static void geometry(const fann_index *ix, uint32_t k, Geom *g)
 }
 
 struct WsLayout {
-    size_t hdr, S, mode, item_start, items, uniq_counts, uniq_ids, total;
+    size_t hdr, S, mode, item_start, items, uniq_counts, part_ok, bucket_cnt, part_ids, uniq_ids, total;
     uint32_t max_items;
 };
 
@@ -95,6 +96,9 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
     w->item_start = o;  o = align_up(o + ((size_t)B + 1) * 4, 256);
     w->items = o;       o = align_up(o + (size_t)w->max_items * 8, 256);
     w->uniq_counts = o; o = align_up(o + (size_t)B * 4, 256);
+    w->part_ok = o;     o = align_up(o + (size_t)B * 4, 256);
+    w->bucket_cnt = o;  o = align_up(o + (size_t)w->max_items * 4, 256);
+    w->part_ids = o;    o = align_up(o + (size_t)total_cands * 8 + 16, 256);      // class buckets, 2 C_b per query
     w->uniq_ids = o;    if (with_uniq) o = align_up(o + (size_t)total_cands * 4 + 16, 256);
     w->total = o;
 }
@@ -137,6 +141,7 @@ extern "C" int fann_create(fann_index **out, int device)
     ix->dedup_smem = (uint32_t)smem_optin;
     if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
+    if (const char *s = getenv("FANN_PARTITION")) ix->partition = atoi(s) != 0;
     if (const char *s = getenv("FANN_L2_FETCH")) {
         int v = atoi(s);
         if (v == 32 || v == 64 || v == 128) CUDA_TRY(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)v));
@@ -359,6 +364,19 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     dp.cand_offsets = (const long long *)cand_offsets; dp.cand_ids = cand_ids; dp.N = ix->N;
     dp.nslots_max = g.nslots_max; dp.hdr = hdr; dp.S = S; dp.mode = mode; dp.item_start = item_start; dp.items = items;
     dp.uniq_ids = uniq_ids; dp.uniq_counts = uniq_counts;
+    dp.part_ids = ix->partition ? (const uint32_t *)(ws + w.part_ids) : nullptr;
+    dp.part_ok = (const uint32_t *)(ws + w.part_ok); dp.bucket_cnt = (const uint32_t *)(ws + w.bucket_cnt);
+    if (timing) cudaEventRecord(ix->ev_dedup[0][0], dstream);
+    if (ix->partition) {
+        PartParams pp;
+        pp.cand_offsets = (const long long *)cand_offsets; pp.cand_ids = cand_ids; pp.N = ix->N;
+        pp.S = S; pp.mode = mode; pp.item_start = item_start;
+        pp.part_ids = (uint32_t *)(ws + w.part_ids); pp.part_ok = (uint32_t *)(ws + w.part_ok);
+        pp.bucket_cnt = (uint32_t *)(ws + w.bucket_cnt);
+        partition_kernel<<<B, kPartThreads, 0, dstream>>>(pp);
+        ix->launches++;
+        CUDA_TRY(cudaGetLastError());
+    }
     ScanParams sp;
     sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
@@ -368,7 +386,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     for (uint32_t c = 0; c < chunks; ++c) {
         const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
         dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
-        if (timing) cudaEventRecord(ix->ev_dedup[c][0], dstream);
+        if (timing && c > 0) cudaEventRecord(ix->ev_dedup[c][0], dstream);
         dedup_kernel<<<ix->num_sms, kDedupThreads, g.dedup_smem, dstream>>>(dp);
         if (timing) cudaEventRecord(ix->ev_dedup[c][1], dstream);
         ix->launches++;

@@ -213,9 +213,11 @@ __global__ void mode_kernel(const long long *__restrict__ cand_offsets, const ui
     const long long Cll = cand_offsets[b + 1] - off0;
     const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;
     uint32_t m = kModeOrdered;
-    if (force < 2) {
+    if (N < 4096) {
+        m = kModeHashed;                                       // ordered classes need N >> S
+    } else if (force < 2) {
         m = force;
-    } else if (C >= 64 && N >= 64) {
+    } else if (C >= 64) {
         const uint32_t *ids = cand_ids + off0;
         const unsigned long long cd = N / (2ull * C);
         const uint32_t close_dist = cd > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)cd;
@@ -257,7 +259,98 @@ struct DedupParams {
     const uint2 *items;                              // [n_items] (query, partition)
     uint32_t *uniq_ids;                              // [total_cands]; query b's list starts at cand_offsets[b]
     uint32_t *uniq_counts;                           // [B], zeroed by plan_kernel
+    const uint32_t *part_ids;                        // [2 * total_cands] buckets written by partition_kernel, or NULL
+    const uint32_t *part_ok;                         // [B] 1: query b's buckets are valid
+    const uint32_t *bucket_cnt;                      // [n_items] IDs in the bucket of each (query, partition) item
 };
+
+// Partition of a query's valid IDs into S classes (both the partition kernel and the dedup kernel's own
+// filter use these, so a class means the same set of IDs wherever it is computed):
+//   ordered  class = floor(id * MS / 2^32), MS = floor(S * 2^32 / N): S contiguous ID ranges of near-equal length;
+//            class p starts at ceil(p * 2^32 / MS)
+//   hashed   class = floor(h1(id) * S / 2^32), h1 the first round of the slot hash
+__device__ __forceinline__ uint32_t ordered_class_mul(uint64_t N, uint32_t S)
+{
+    return (uint32_t)(((unsigned long long)S << 32) / N);      // S < N (mode_kernel sends tiny N to hashed mode)
+}
+__device__ __forceinline__ uint32_t ordered_class_start(uint32_t MS, uint32_t cls, uint64_t N)
+{
+    const unsigned long long v = (((unsigned long long)cls << 32) + MS - 1) / MS;
+    return (uint32_t)(v < N ? v : N);
+}
+__device__ __forceinline__ uint32_t hash_round1(uint32_t x) { return (x ^ (x >> 16)) * 0x7feb352dU; }
+
+__device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, uint32_t C);
+
+constexpr uint32_t kMaxPartBuckets = 8;              // partition_kernel handles 2..8 classes per query
+constexpr int kPartThreads = 512;
+
+struct PartParams {
+    const long long *cand_offsets;
+    const uint32_t *cand_ids;
+    uint64_t N;
+    const uint32_t *S, *mode, *item_start;
+    uint32_t *part_ids;                              // query b's buckets at 2 * cand_offsets[b], bucket p at p * cap_b
+    uint32_t *part_ok;                               // [B]
+    uint32_t *bucket_cnt;                            // [n_items]
+};
+
+// Splits the candidate list of every query that needs S >= 2 dedup partitions into its S classes, so that
+// each dedup pass reads only its own IDs instead of filtering the whole list S times.  One CTA per query.
+// Bucket p of query b holds at most cap_b = 2 C_b / S_b IDs (twice its fair share); if a class is larger
+// (bunched IDs) part_ok[b] stays 0 and the dedup kernel filters the original list itself.
+__global__ void __launch_bounds__(kPartThreads) partition_kernel(const PartParams p)
+{
+    __shared__ uint32_t scnt[kMaxPartBuckets];
+    const uint32_t b = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const uint32_t S = p.S[b];
+    if (S < 2 || S > kMaxPartBuckets) { if (tid == 0) p.part_ok[b] = 0; return; }
+    const bool hashed = p.mode[b] == kModeHashed;
+    const long long off0 = p.cand_offsets[b];
+    const long long Cll = p.cand_offsets[b + 1] - off0;
+    const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;
+    const uint32_t capb = (uint32_t)(2ull * C / S);
+    const uint32_t MS = hashed ? 0u : ordered_class_mul(p.N, S);
+    uint32_t *out = p.part_ids + 2 * off0;
+    if (tid < kMaxPartBuckets) scnt[tid] = 0;
+    __syncthreads();
+    const uint32_t *ids = p.cand_ids + off0;
+    const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
+    const uint32_t nvec = (C + shift + 3u) >> 2;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    bool overflow = false;
+    for (uint32_t vb = 0; vb < nvec; vb += kPartThreads) {     // uniform trip count: ballots below need whole warps
+        const uint32_t v = vb + tid;
+        uint4 q4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+        if (v < nvec) q4 = load_ids4(ids, 4ll * v - shift, C);
+        const uint32_t x[4] = {q4.x, q4.y, q4.z, q4.w};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const bool valid = (uint64_t)x[e] < p.N;           // also drops kIdNone
+            uint32_t cls = hashed ? __umulhi(hash_round1(x[e]), S) : __umulhi(x[e], MS);
+            if (!valid) cls = 0xFFu;
+            uint32_t own = 0, mine_bal = 0;
+#pragma unroll
+            for (uint32_t q = 0; q < kMaxPartBuckets; ++q) {
+                if (q >= S) break;
+                const uint32_t bal = __ballot_sync(0xffffffffu, cls == q);
+                if (cls == q) own = bal;
+                if (lane == q) mine_bal = bal;
+            }
+            uint32_t base = 0;
+            if (lane < S && mine_bal) base = atomicAdd(&scnt[lane], (uint32_t)__popc(mine_bal));
+            base = __shfl_sync(0xffffffffu, base, cls & 31u);
+            const uint32_t pos = base + __popc(own & lt_mask);
+            if (valid) {
+                if (pos < capb) out[(size_t)cls * capb + pos] = x[e];
+                else overflow = true;
+            }
+        }
+    }
+    const bool bad = __syncthreads_or(overflow);
+    if (tid < S) p.bucket_cnt[p.item_start[b] + tid] = scnt[tid] < capb ? scnt[tid] : capb;
+    if (tid == 0) p.part_ok[b] = bad ? 0u : 1u;
+}
 
 // Elements e0 .. e0+3 of a candidate list of C IDs (e0 may be negative or reach past the end at the
 // two ragged ends of a list); positions outside [0, C) read as kIdNone.  ids + e0 is 16-byte aligned.
@@ -315,17 +408,23 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
         const long long Cll = p.cand_offsets[b + 1] - off0;
         const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;       // plan guarantees C / S <= 0.75 nslots_max
 
+        // pre-partitioned: this item's IDs were split off by partition_kernel; every ID read is ours
+        const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
+        const uint32_t Cin = pre ? p.bucket_cnt[item] : C;     // IDs this pass reads
+
         // table sized to the partition: 2 slots per candidate, never more than the CTA can hold
         uint32_t nslots = p.nslots_max;
         {
-            const unsigned long long want = ((unsigned long long)(C / S + 1) * 2 + 128) & ~3ull;
+            const unsigned long long want = ((unsigned long long)(pre ? Cin : C / S + 1) * 2 + 128) & ~3ull;
             if (want < nslots) nslots = (uint32_t)want;
         }
-        // ordered mode: this partition owns IDs in [lo, lo + span); slot = (id - lo) * nslots / span
-        uint32_t lo = 0, span = 0, slot_mul = 0;
+        // ordered mode: this partition owns the IDs of class `part`, a range [lo, lo + span);
+        // slot = (id - lo) * nslots / span
+        uint32_t lo = 0, span = 0, slot_mul = 0, class_mul = 0;
         if (!hashed) {
-            const unsigned long long l = p.N * part / S, h = p.N * (part + 1ull) / S;
-            lo = (uint32_t)l; span = (uint32_t)(h - l);
+            class_mul = ordered_class_mul(p.N, S);
+            lo = ordered_class_start(class_mul, part, p.N);
+            span = ordered_class_start(class_mul, part + 1, p.N) - lo;
             slot_mul = span > nslots ? (uint32_t)(((unsigned long long)nslots << 32) / span) : 0u;   // 0: slot = id - lo
         }
         {
@@ -336,21 +435,21 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 
         // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list.
         // Vectors [v_in0, v_in1) lie wholly inside the list and are read with one 16-byte load.
-        const uint32_t *ids = p.cand_ids + off0;
+        const uint32_t *ids = pre ? p.part_ids + 2 * off0 + (size_t)part * (uint32_t)(2ull * C / S) : p.cand_ids + off0;
         const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
         const uint4 *ids4 = reinterpret_cast<const uint4 *>(ids - shift);
-        const uint32_t nvec = C ? (C + shift + 3u) >> 2 : 0u;
-        const uint32_t v_in0 = shift ? 1u : 0u, v_in1 = (C + shift) >> 2;
+        const uint32_t nvec = Cin ? (Cin + shift + 3u) >> 2 : 0u;
+        const uint32_t v_in0 = shift ? 1u : 0u, v_in1 = (Cin + shift) >> 2;
         const uint4 none4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
         auto load_vec = [&](uint32_t v) -> uint4 {
             if (v >= v_in0 && v < v_in1) return __ldg(ids4 + v);
-            if (v < nvec) return load_ids4(ids, 4ll * v - shift, C);
+            if (v < nvec) return load_ids4(ids, 4ll * v - shift, Cin);
             return none4;
         };
         // shared-memory byte address of the home slot of a valid ID of this partition
         auto place = [&](uint32_t x) -> uint32_t {
             if (!hashed) return tbl + ((slot_mul ? __umulhi(x - lo, slot_mul) : x - lo) << 2);
-            uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
+            uint32_t a = hash_round1(x);
             a = (a ^ (a >> 15)) * 0x846ca68bU;
             a ^= a >> 16;
             return tbl + (__umulhi(a, nslots) << 2);
@@ -374,9 +473,11 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
             if (!hashed) {
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
-                    const uint32_t x = id[j] - lo;             // kIdNone and IDs >= N fall outside every span
+                    const uint32_t x = id[j] - lo;
                     const uint32_t a = tbl + ((slot_mul ? __umulhi(x, slot_mul) : x) << 2);
-                    const bool mine = x < span;
+                    // a pre-partitioned bucket holds only this class; else: class test (x < span) drops
+                    // other classes, IDs >= N and kIdNone (lo + span <= N)
+                    const bool mine = pre ? id[j] != kIdNone : x < span;
                     sa[j] = mine ? a : none_addr;
                     if (!mine) id[j] = kIdNone;
                 }
@@ -384,8 +485,8 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j];
-                    const uint32_t a = (x ^ (x >> 16)) * 0x7feb352dU;
-                    const bool mine = x != kIdNone && (uint64_t)x < p.N && (S == 1 || __umulhi(a, S) == part);
+                    const bool mine = pre ? x != kIdNone
+                                          : ((uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part));
                     sa[j] = mine ? place(x) : none_addr;
                     if (!mine) id[j] = kIdNone;
                 }
