@@ -21,6 +21,7 @@ struct fann_index {
     int smem_optin = 0;                    // max dynamic shared memory per block
     uint32_t chunks = 1;                   // batch chunks: dedup of chunk i+1 runs beside the scan of chunk i
     uint32_t force_mode = 2;               // dedup placement: 0 ordered, 1 hashed, 2 decided per query (FANN_DEDUP_MODE)
+    uint32_t scan_ring = 3;                // scan kernel: stages of the per-warp code-row ring, 0 = rows through registers (FANN_SCAN_RING)
     bool partition = true;                 // split lists into their dedup classes first (FANN_PARTITION=0: filter per pass)
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint64_t launches = 0;
@@ -68,7 +69,7 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Geom {
     uint32_t nslots_max, cap_c, dedup_smem;          // dedup: table slots per CTA, candidates per partition
-    uint32_t cap, scan_smem;                         // scan: candidate-buffer keys, shared memory per CTA
+    uint32_t cap, scan_smem, ring;                   // scan: candidate-buffer keys, shared memory per CTA, ring depth
 };
 
 static void geometry(const fann_index *ix, uint32_t k, Geom *g)
@@ -76,8 +77,9 @@ static void geometry(const fann_index *ix, uint32_t k, Geom *g)
     g->dedup_smem = ix->dedup_smem;
     g->nslots_max = ((g->dedup_smem - kDedupTableOff) / 4) & ~3u;
     g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
-    g->cap = k <= 256 ? 4096u : 8192u;
-    g->scan_smem = (uint32_t)scan_smem_bytes(g->cap);
+    g->ring = ix->scan_ring;
+    g->cap = (k <= 256 || g->ring) ? 4096u : 8192u;            // the ring takes the shared memory of the larger buffer
+    g->scan_smem = (uint32_t)scan_smem_bytes(g->cap, g->ring);
 }
 
 struct WsLayout {
@@ -108,10 +110,10 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
 extern "C" const char *fann_last_error(void) { return g_err; }
 extern "C" const char *fann_version(void) { return "fann 0.2 sm_100a"; }
 
-template <int G, int NB>
+template <int G, int NB, int D>
 static cudaError_t set_scan_attr(int smem)
 {
-    return cudaFuncSetAttribute(scan_kernel<G, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    return cudaFuncSetAttribute(scan_kernel<G, NB, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
 extern "C" int fann_create(fann_index **out, int device)
@@ -133,15 +135,23 @@ extern "C" int fann_create(fann_index **out, int device)
         return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
                     smem_optin, scan_max);
     CUDA_TRY(cudaFuncSetAttribute(dedup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
-    CUDA_TRY((set_scan_attr<1, 4>(scan_max)));
-    CUDA_TRY((set_scan_attr<2, 4>(scan_max)));
-    CUDA_TRY((set_scan_attr<4, 2>(scan_max)));
+    const int ring_max = (int)scan_smem_bytes(4096, 3);
+    if (ring_max > smem_optin)
+        return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
+                    smem_optin, ring_max);
+    CUDA_TRY((set_scan_attr<1, 4, 0>(scan_max)));
+    CUDA_TRY((set_scan_attr<2, 4, 0>(scan_max)));
+    CUDA_TRY((set_scan_attr<4, 2, 0>(scan_max)));
+    CUDA_TRY((set_scan_attr<1, 4, 3>(ring_max)));
+    CUDA_TRY((set_scan_attr<2, 4, 3>(ring_max)));
+    CUDA_TRY((set_scan_attr<4, 2, 3>(ring_max)));
     fann_index *ix = new fann_index();
     ix->device = device; ix->num_sms = num_sms; ix->smem_optin = smem_optin;
     ix->dedup_smem = (uint32_t)smem_optin;
     if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
     if (const char *s = getenv("FANN_PARTITION")) ix->partition = atoi(s) != 0;
+    if (const char *s = getenv("FANN_SCAN_RING")) { int v = atoi(s); if (v == 0 || v == 3) ix->scan_ring = (uint32_t)v; }
     if (const char *s = getenv("FANN_L2_FETCH")) {
         int v = atoi(s);
         if (v == 32 || v == 64 || v == 128) CUDA_TRY(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)v));
@@ -295,10 +305,14 @@ extern "C" size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_
 
 static cudaError_t launch_scan(const fann_index *ix, int grid, size_t smem, cudaStream_t stream, const ScanParams &p)
 {
-    switch (ix->row_bytes) {
-    case 16: scan_kernel<1, 4><<<grid, kScanThreads, smem, stream>>>(p); break;
-    case 32: scan_kernel<2, 4><<<grid, kScanThreads, smem, stream>>>(p); break;
-    default: scan_kernel<4, 2><<<grid, kScanThreads, smem, stream>>>(p); break;
+    if (ix->scan_ring) switch (ix->row_bytes) {
+    case 16: scan_kernel<1, 4, 3><<<grid, kScanThreads, smem, stream>>>(p); break;
+    case 32: scan_kernel<2, 4, 3><<<grid, kScanThreads, smem, stream>>>(p); break;
+    default: scan_kernel<4, 2, 3><<<grid, kScanThreads, smem, stream>>>(p); break;
+    } else switch (ix->row_bytes) {
+    case 16: scan_kernel<1, 4, 0><<<grid, kScanThreads, smem, stream>>>(p); break;
+    case 32: scan_kernel<2, 4, 0><<<grid, kScanThreads, smem, stream>>>(p); break;
+    default: scan_kernel<4, 2, 0><<<grid, kScanThreads, smem, stream>>>(p); break;
     }
     return cudaGetLastError();
 }
@@ -307,10 +321,14 @@ static int scan_ctas_per_sm(const fann_index *ix, size_t smem)
 {
     int n = 0;
     cudaError_t e;
-    switch (ix->row_bytes) {
-    case 16: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<1, 4>, kScanThreads, smem); break;
-    case 32: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<2, 4>, kScanThreads, smem); break;
-    default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<4, 2>, kScanThreads, smem); break;
+    if (ix->scan_ring) switch (ix->row_bytes) {
+    case 16: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<1, 4, 3>, kScanThreads, smem); break;
+    case 32: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<2, 4, 3>, kScanThreads, smem); break;
+    default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<4, 2, 3>, kScanThreads, smem); break;
+    } else switch (ix->row_bytes) {
+    case 16: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<1, 4, 0>, kScanThreads, smem); break;
+    case 32: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<2, 4, 0>, kScanThreads, smem); break;
+    default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, scan_kernel<4, 2, 0>, kScanThreads, smem); break;
     }
     return (e == cudaSuccess && n >= 1) ? n : 1;
 }

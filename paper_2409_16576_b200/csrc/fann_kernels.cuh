@@ -58,6 +58,21 @@ __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
     asm volatile("st.shared.u32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
 }
 
+__device__ __forceinline__ uint4 lds_u128(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+// 16-byte asynchronous copy global -> shared (LDGSTS), 64-byte L2 fetch; completes in commit-group order.
+__device__ __forceinline__ void cp_async_16(uint32_t saddr, const void *g)
+{
+    asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" :: "r"(saddr), "l"(g) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+
 // Block-wide bitonic sort (ascending) of n = 2^p keys in shared memory,
 // starting from sorted runs of length first_size / 2.
 __device__ __forceinline__ void bitonic_sort_smem(unsigned long long *a, uint32_t n, uint32_t first_size)
@@ -619,7 +634,11 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 //   [3136, +cap*8)       top-k candidate buffer, 64-bit keys (dist bits << 32 | id)
 //   [.., +64 KB)         lookup table of the query, c-major: entry (c, col) at byte c*256 + col*4
 constexpr uint32_t kScanBufOff = 64 + kSample * 8 + kSample * 4;
-__host__ __device__ inline size_t scan_smem_bytes(uint32_t cap) { return kScanBufOff + (size_t)cap * 8 + 65536; }
+constexpr uint32_t kRingStageBytes = 2048 + 512;     // 2 KB of code rows + the stage's IDs (32 .. 128 of them)
+__host__ __device__ inline size_t scan_smem_bytes(uint32_t cap, uint32_t ring_depth = 0)
+{
+    return kScanBufOff + (size_t)cap * 8 + 65536 + (size_t)ring_depth * kScanWarps * kRingStageBytes;
+}
 
 struct ScanParams {
     const uint8_t *codes;                            // [N][16*G], library copy
@@ -755,7 +774,10 @@ __device__ __forceinline__ float adc16(const uint4 r, const unsigned char *lutb,
     return (acc[0] + acc[1]) + (acc[2] + acc[3]);
 }
 
-template <int G, int NB>
+// D = 0: code rows go through registers (NB row groups in flight per lane).  D >= 2: every warp keeps a
+// private ring of D stages in shared memory and fills it D - 1 stages ahead with 16-byte asynchronous
+// copies, so row reads stay in flight while the warp computes.
+template <int G, int NB, int D>
 __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 {
     constexpr int ROWB = 16 * G;
@@ -791,7 +813,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
         const uint32_t beta = (uint32_t)j ^ x0;
         sel[j] = (4u + beta) | (beta << 4) | ((8u | (4u + beta)) << 8) | ((8u | (4u + beta)) << 12);
     }
-    const uint32_t margin = kScanWarps * 32 * NB + 64;         // keys appended between the buffer passing its limit and the prune
+    constexpr int NBS = 4 / G;                                 // ring: IDs per lane per stage (a stage is 2 KB of rows)
+    const uint32_t margin = kScanWarps * 32 * (D ? NBS : NB) + 64;   // keys appended between the buffer passing its limit and the prune
     const uint32_t limit = p.cap - margin;
 
     for (;;) {
@@ -819,60 +842,138 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
         }
         __syncthreads();
 
-        const uint32_t per_iter = kScanWarps * 32 * NB;
-        const uint32_t n_iter = (U + per_iter - 1) / per_iter;
-        // Warps run free: no barrier per iteration.  The warp whose append takes the buffer past its limit
-        // raises misc[9]; every warp sees it before its next iteration (each appends at most one more
-        // iteration's keys, which the margin above the limit holds) and meets the others at the barrier
-        // below, where the buffer is pruned.  A warp out of work waits there too, so the barrier completes
-        // exactly when every warp is done or has seen the flag.
-        uint32_t itn = 0;
-        for (;;) {
-          while (itn < n_iter && !vm[9]) {
-            const uint32_t base = (itn * kScanWarps + warp) * 32 * NB;
-            ++itn;
-            if (base < U) {
-                uint32_t id[NB];
+        if constexpr (D > 0) {
+            const uint32_t ring = (uint32_t)__cvta_generic_to_shared(lutb + 65536) + warp * (D * kRingStageBytes);
+            const uint32_t per_stage = 32 * NBS;
+            const uint32_t n_st = (U + kScanWarps * per_stage - 1) / (kScanWarps * per_stage);   // stages per warp
+            uint32_t idn[NBS];                                 // IDs of the next stage to issue, loaded one stage ahead
+            auto load_ids = [&](uint32_t st) {
+                const uint32_t base = (st * kScanWarps + warp) * per_stage;
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb) {
+                for (int nb = 0; nb < NBS; ++nb) {
                     const uint32_t idx = base + nb * 32 + lane;
-                    id[nb] = idx < U ? __ldg(uq + idx) : kIdNone;
+                    idn[nb] = idx < U ? __ldg(uq + idx) : kIdNone;
                 }
-                uint4 rw[NB][G];
+            };
+            // start the copies of stage st (its IDs are in idn), then fetch the IDs of stage st + 1
+            auto issue = [&](uint32_t st) {
+                if (st < n_st && (st * kScanWarps + warp) * per_stage < U) {
+                    const uint32_t sa = ring + (st % D) * kRingStageBytes;
 #pragma unroll
-                for (int nb = 0; nb < NB; ++nb)
+                    for (int nb = 0; nb < NBS; ++nb) {
+                        sts_u32(sa + 2048 + (nb * 32 + lane) * 4, idn[nb]);
 #pragma unroll
-                    for (int t = 0; t < G; ++t) {
-                        uint32_t rid = G == 1 ? id[nb] : __shfl_sync(0xffffffffu, id[nb], (lane & ~(G - 1)) | t);
-                        if (rid == kIdNone) rid = 0;
-                        rw[nb][t] = ldg_nc_16(p.codes + (uint64_t)rid * ROWB + q * 16);
+                        for (int t = 0; t < G; ++t) {
+                            uint32_t rid = G == 1 ? idn[nb] : __shfl_sync(0xffffffffu, idn[nb], (lane & ~(G - 1)) | t);
+                            if (rid == kIdNone) rid = 0;
+                            cp_async_16(sa + (nb * 32 + (lane & ~(G - 1)) + t) * ROWB + q * 16,
+                                        p.codes + (uint64_t)rid * ROWB + q * 16);
+                        }
                     }
-                const unsigned long long tau = *reinterpret_cast<volatile unsigned long long *>(tau_p);
-#pragma unroll
-                for (int nb = 0; nb < NB; ++nb) {
-                    float mine = 0.f;
-#pragma unroll
-                    for (int t = 0; t < G; ++t) {
-                        float s = adc16<G>(rw[nb][t], lutb, Bw, sel, swap1, swap2);
-                        if (G >= 2) s += __shfl_xor_sync(0xffffffffu, s, 1);
-                        if (G == 4) s += __shfl_xor_sync(0xffffffffu, s, 2);
-                        if (q == (uint32_t)t) mine = s;
-                    }
-                    const unsigned long long key = ((unsigned long long)__float_as_uint(mine) << 32) | id[nb];
-                    const bool keep = id[nb] != kIdNone && key < tau;
-                    const uint32_t bal = __ballot_sync(0xffffffffu, keep);
-                    if (bal) {
-                        uint32_t pos = 0;
-                        if (lane == 0) pos = atomicAdd(&misc[0], (uint32_t)__popc(bal));
-                        pos = __shfl_sync(0xffffffffu, pos, 0);
-                        if (keep) buf[pos + __popc(bal & lt_mask)] = key;
-                    }
+                    load_ids(st + 1);
                 }
-                if (lane == 0 && vm[0] > limit) vm[9] = 1;
+                cp_async_commit();                             // one group per stage, empty past the end
+            };
+            load_ids(0);
+#pragma unroll
+            for (int d = 0; d < D - 1; ++d) issue(d);
+            uint32_t st = 0;
+            for (;;) {
+                while (st < n_st && !vm[9]) {
+                    issue(st + D - 1);
+                    cp_async_wait<D - 1>();                    // stage st has landed (this lane's copies)
+                    __syncwarp();                              // ... and every other lane's
+                    if ((st * kScanWarps + warp) * per_stage < U) {
+                        const uint32_t sa = ring + (st % D) * kRingStageBytes;
+                        const unsigned long long tau = *reinterpret_cast<volatile unsigned long long *>(tau_p);
+#pragma unroll
+                        for (int nb = 0; nb < NBS; ++nb) {
+                            float mine = 0.f;
+#pragma unroll
+                            for (int t = 0; t < G; ++t) {
+                                const uint4 rw = lds_u128(sa + (nb * 32 + (lane & ~(G - 1)) + t) * ROWB + q * 16);
+                                float sum = adc16<G>(rw, lutb, Bw, sel, swap1, swap2);
+                                if (G >= 2) sum += __shfl_xor_sync(0xffffffffu, sum, 1);
+                                if (G == 4) sum += __shfl_xor_sync(0xffffffffu, sum, 2);
+                                if (q == (uint32_t)t) mine = sum;
+                            }
+                            const uint32_t idv = lds_u32(sa + 2048 + (nb * 32 + lane) * 4);
+                            const unsigned long long key = ((unsigned long long)__float_as_uint(mine) << 32) | idv;
+                            const bool keep = idv != kIdNone && key < tau;
+                            const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+                            if (bal) {
+                                uint32_t pos = 0;
+                                if (lane == 0) pos = atomicAdd(&misc[0], (uint32_t)__popc(bal));
+                                pos = __shfl_sync(0xffffffffu, pos, 0);
+                                if (keep) buf[pos + __popc(bal & lt_mask)] = key;
+                            }
+                        }
+                        if (lane == 0 && vm[0] > limit) vm[9] = 1;
+                    }
+                    __syncwarp();                              // the stage's slot is refilled by the next issue
+                    ++st;
+                }
+                if (!__syncthreads_or(vm[9] != 0)) break;
+                prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
             }
-          }
-          if (!__syncthreads_or(vm[9] != 0)) break;
-          prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
+            cp_async_wait<0>();
+        } else {
+            const uint32_t per_iter = kScanWarps * 32 * NB;
+            const uint32_t n_iter = (U + per_iter - 1) / per_iter;
+            // Warps run free: no barrier per iteration.  The warp whose append takes the buffer past its limit
+            // raises misc[9]; every warp sees it before its next iteration (each appends at most one more
+            // iteration's keys, which the margin above the limit holds) and meets the others at the barrier
+            // below, where the buffer is pruned.  A warp out of work waits there too, so the barrier completes
+            // exactly when every warp is done or has seen the flag.
+            uint32_t itn = 0;
+            for (;;) {
+              while (itn < n_iter && !vm[9]) {
+                const uint32_t base = (itn * kScanWarps + warp) * 32 * NB;
+                ++itn;
+                if (base < U) {
+                    uint32_t id[NB];
+    #pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) {
+                        const uint32_t idx = base + nb * 32 + lane;
+                        id[nb] = idx < U ? __ldg(uq + idx) : kIdNone;
+                    }
+                    uint4 rw[NB][G];
+    #pragma unroll
+                    for (int nb = 0; nb < NB; ++nb)
+    #pragma unroll
+                        for (int t = 0; t < G; ++t) {
+                            uint32_t rid = G == 1 ? id[nb] : __shfl_sync(0xffffffffu, id[nb], (lane & ~(G - 1)) | t);
+                            if (rid == kIdNone) rid = 0;
+                            rw[nb][t] = ldg_nc_16(p.codes + (uint64_t)rid * ROWB + q * 16);
+                        }
+                    const unsigned long long tau = *reinterpret_cast<volatile unsigned long long *>(tau_p);
+    #pragma unroll
+                    for (int nb = 0; nb < NB; ++nb) {
+                        float mine = 0.f;
+    #pragma unroll
+                        for (int t = 0; t < G; ++t) {
+                            float s = adc16<G>(rw[nb][t], lutb, Bw, sel, swap1, swap2);
+                            if (G >= 2) s += __shfl_xor_sync(0xffffffffu, s, 1);
+                            if (G == 4) s += __shfl_xor_sync(0xffffffffu, s, 2);
+                            if (q == (uint32_t)t) mine = s;
+                        }
+                        const unsigned long long key = ((unsigned long long)__float_as_uint(mine) << 32) | id[nb];
+                        const bool keep = id[nb] != kIdNone && key < tau;
+                        const uint32_t bal = __ballot_sync(0xffffffffu, keep);
+                        if (bal) {
+                            uint32_t pos = 0;
+                            if (lane == 0) pos = atomicAdd(&misc[0], (uint32_t)__popc(bal));
+                            pos = __shfl_sync(0xffffffffu, pos, 0);
+                            if (keep) buf[pos + __popc(bal & lt_mask)] = key;
+                        }
+                    }
+                    if (lane == 0 && vm[0] > limit) vm[9] = 1;
+                }
+              }
+              if (!__syncthreads_or(vm[9] != 0)) break;
+              prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
+            }
+
         }
 
         // exact top-k of what is left
