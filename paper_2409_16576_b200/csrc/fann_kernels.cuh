@@ -866,7 +866,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                         for (int t = 0; t < G; ++t) {
                             uint32_t rid = G == 1 ? idn[nb] : __shfl_sync(0xffffffffu, idn[nb], (lane & ~(G - 1)) | t);
                             if (rid == kIdNone) rid = 0;
-                            cp_async_16(sa + (nb * 32 + (lane & ~(G - 1)) + t) * ROWB + q * 16,
+                            // rows read together (same t) sit together: slot = t * (32 / G) + lane / G
+                            cp_async_16(sa + (nb * 32 + t * (32 / G) + r) * ROWB + q * 16,
                                         p.codes + (uint64_t)rid * ROWB + q * 16);
                         }
                     }
@@ -891,7 +892,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                             float mine = 0.f;
 #pragma unroll
                             for (int t = 0; t < G; ++t) {
-                                const uint4 rw = lds_u128(sa + (nb * 32 + (lane & ~(G - 1)) + t) * ROWB + q * 16);
+                                const uint4 rw = lds_u128(sa + (nb * 32 + t * (32 / G) + r) * ROWB + q * 16);
                                 float sum = adc16<G>(rw, lutb, Bw, sel, swap1, swap2);
                                 if (G >= 2) sum += __shfl_xor_sync(0xffffffffu, sum, 1);
                                 if (G == 4) sum += __shfl_xor_sync(0xffffffffu, sum, 2);
