@@ -334,10 +334,17 @@ __global__ void __launch_bounds__(kPartThreads) partition_kernel(const PartParam
     const uint32_t nvec = (C + shift + 3u) >> 2;
     const uint32_t lt_mask = (1u << lane) - 1u;
     bool overflow = false;
+    const uint4 *ids4 = reinterpret_cast<const uint4 *>(ids - shift);
+    const uint32_t v_in0 = shift ? 1u : 0u, v_in1 = (C + shift) >> 2;      // vectors wholly inside the list
+    auto load_vec = [&](uint32_t v) -> uint4 {
+        if (v >= v_in0 && v < v_in1) return __ldg(ids4 + v);
+        if (v < nvec) return load_ids4(ids, 4ll * v - shift, C);
+        return make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+    };
+    uint4 nxt = load_vec(tid);
     for (uint32_t vb = 0; vb < nvec; vb += kPartThreads) {     // uniform trip count: ballots below need whole warps
-        const uint32_t v = vb + tid;
-        uint4 q4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
-        if (v < nvec) q4 = load_ids4(ids, 4ll * v - shift, C);
+        const uint4 q4 = nxt;
+        nxt = load_vec(vb + kPartThreads + tid);               // one iteration ahead
         const uint32_t x[4] = {q4.x, q4.y, q4.z, q4.w};
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -490,9 +497,9 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                 for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j] - lo;
                     const uint32_t a = tbl + ((slot_mul ? __umulhi(x, slot_mul) : x) << 2);
-                    // a pre-partitioned bucket holds only this class; else: class test (x < span) drops
-                    // other classes, IDs >= N and kIdNone (lo + span <= N)
-                    const bool mine = pre ? id[j] != kIdNone : x < span;
+                    // class test: drops other classes, IDs >= N and kIdNone (lo + span <= N); a
+                    // pre-partitioned bucket holds only this class, so there it drops just the padding
+                    const bool mine = x < span;
                     sa[j] = mine ? a : none_addr;
                     if (!mine) id[j] = kIdNone;
                 }
@@ -500,8 +507,7 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j];
-                    const bool mine = pre ? x != kIdNone
-                                          : ((uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part));
+                    const bool mine = (uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part);
                     sa[j] = mine ? place(x) : none_addr;
                     if (!mine) id[j] = kIdNone;
                 }
