@@ -351,17 +351,13 @@ __global__ void __launch_bounds__(kPartThreads) partition_kernel(const PartParam
             const bool valid = (uint64_t)x[e] < p.N;           // also drops kIdNone
             uint32_t cls = hashed ? __umulhi(hash_round1(x[e]), S) : __umulhi(x[e], MS);
             if (!valid) cls = 0xFFu;
-            uint32_t own = 0, mine_bal = 0;
-#pragma unroll
-            for (uint32_t q = 0; q < kMaxPartBuckets; ++q) {
-                if (q >= S) break;
-                const uint32_t bal = __ballot_sync(0xffffffffu, cls == q);
-                if (cls == q) own = bal;
-                if (lane == q) mine_bal = bal;
-            }
+            // lanes of the same class: one MATCH instead of a ballot per class; the lowest lane of each
+            // class reserves the class's output range for all of them
+            const uint32_t own = __match_any_sync(0xffffffffu, cls);
+            const uint32_t leader = __ffs(own) - 1;
             uint32_t base = 0;
-            if (lane < S && mine_bal) base = atomicAdd(&scnt[lane], (uint32_t)__popc(mine_bal));
-            base = __shfl_sync(0xffffffffu, base, cls & 31u);
+            if (valid && lane == leader) base = atomicAdd(&scnt[cls], (uint32_t)__popc(own));
+            base = __shfl_sync(0xffffffffu, base, leader);
             const uint32_t pos = base + __popc(own & lt_mask);
             if (valid) {
                 if (pos < capb) out[(size_t)cls * capb + pos] = x[e];
@@ -434,10 +430,11 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
         const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
         const uint32_t Cin = pre ? p.bucket_cnt[item] : C;     // IDs this pass reads
 
-        // table sized to the partition: 2 slots per candidate, never more than the CTA can hold
+        // table sized to the partition, never more than the CTA can hold
         uint32_t nslots = p.nslots_max;
         {
-            const unsigned long long want = ((unsigned long long)(pre ? Cin : C / S + 1) * 2 + 128) & ~3ull;
+            // 2 slots per expected candidate; 1.5 where the count is exact (about 0.4 full after dedup)
+            const unsigned long long want = ((pre ? (unsigned long long)Cin * 3 / 2 : (unsigned long long)(C / S + 1) * 2) + 128) & ~3ull;
             if (want < nslots) nslots = (uint32_t)want;
         }
         // ordered mode: this partition owns the IDs of class `part`, a range [lo, lo + span);
@@ -609,24 +606,21 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                 if (lane == 31) misc[1] = incl ? atomicAdd(p.uniq_counts + b, incl) : 0u;
             }
             __syncthreads();
-            uint32_t *out = p.uniq_ids + off0 + misc[1];
-            uint32_t run = wsum[warp];
+            // 128 slots per warp step, written word-plane by word-plane (slots 4l of all lanes, then 4l+1, ...):
+            // ascending between steps, a fixed shuffle inside one -- four ballots instead of a warp scan
+            uint32_t *out = p.uniq_ids + off0 + misc[1] + wsum[warp];
+            const uint32_t lt_mask = (1u << lane) - 1u;
             for (uint32_t vb = v0; vb < v1; vb += 32) {
                 const uint32_t v = vb + lane;
                 const uint4 t = v < v1 ? t4[v] : make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
-                const uint32_t cnt = (t.x != kEmpty) + (t.y != kEmpty) + (t.z != kEmpty) + (t.w != kEmpty);
-                uint32_t incl = cnt;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += u;
-                }
-                uint32_t pos = run + incl - cnt;
-                if (t.x != kEmpty) out[pos++] = t.x;
-                if (t.y != kEmpty) out[pos++] = t.y;
-                if (t.z != kEmpty) out[pos++] = t.z;
-                if (t.w != kEmpty) out[pos++] = t.w;
-                run += __shfl_sync(0xffffffffu, incl, 31);
+                const uint32_t b0 = __ballot_sync(0xffffffffu, t.x != kEmpty), b1 = __ballot_sync(0xffffffffu, t.y != kEmpty);
+                const uint32_t b2 = __ballot_sync(0xffffffffu, t.z != kEmpty), b3 = __ballot_sync(0xffffffffu, t.w != kEmpty);
+                const uint32_t c1 = __popc(b0), c2 = c1 + __popc(b1), c3 = c2 + __popc(b2);
+                if (t.x != kEmpty) out[__popc(b0 & lt_mask)] = t.x;
+                if (t.y != kEmpty) out[c1 + __popc(b1 & lt_mask)] = t.y;
+                if (t.z != kEmpty) out[c2 + __popc(b2 & lt_mask)] = t.z;
+                if (t.w != kEmpty) out[c3 + __popc(b3 & lt_mask)] = t.w;
+                out += c3 + __popc(b3);
             }
         }
     }

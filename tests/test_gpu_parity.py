@@ -133,8 +133,8 @@ def test_lut_query_on_centroid_is_exact_zero(fann, tiny):
 # ------------------------------------------------------------------ (5) dedup
 
 def _dedup_check(fann, w, off, ids, ascending=None):
-    """ascending: query indices whose distinct list must come out non-decreasing (one partition,
-    ordered placement) except for the few IDs displaced by probing."""
+    """ascending: query indices whose distinct list must come out in ascending order (one partition,
+    ordered placement) up to the shuffle inside a compaction step and the few IDs displaced by probing."""
     ix = fann.FannIndex(0)
     ix.load_codes(w.codes.to(DEV))
     o = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int64)).to(DEV)
@@ -148,8 +148,9 @@ def _dedup_check(fann, w, off, ids, ascending=None):
         assert ucnt[b] == want.size, f"query {b}: {ucnt[b]} != {want.size}"
         assert np.array_equal(np.sort(got), want), f"query {b}: distinct sets differ"
         if ascending and b in ascending and got.size > 1:
-            inversions = np.count_nonzero(np.diff(got.astype(np.int64)) < 0)
-            assert inversions <= 0.25 * got.size, f"query {b}: {inversions} descents in {got.size} ids"
+            g64 = got.astype(np.int64)                         # ascending beyond the 128-slot compaction step
+            far = np.count_nonzero(g64[512:] < g64[:-512])
+            assert far <= 0.01 * got.size, f"query {b}: {far} of {got.size} ids descend over a distance of 512"
 
 
 def test_dedup_sets_bit_exact(fann, tiny_local, w_int, w_k1000):
