@@ -241,9 +241,10 @@ def main():
     achieved = algo_bytes / (scan_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "scan_kernel", "achieved": round(achieved, 1), "peak": peak,
                 "unit": "GB/s", "frac": round(achieved / peak, 4),
-                # dram__bytes_read+write per gathered row from the committed ncu --set full capture of this kernel
-                # (profiles/r1e_scan_kernel_rows64_ncu.txt, 64-byte rows), scaled to this launch; null for other rows
-                "traffic": int(68.5 * U_total) if M > 32 else None,
+                # dram__bytes_read+write of this kernel per gathered row, measured by ncu on this very workload
+                # (profiles/r1j_launches_u8_1b_m64.md: 50.56 GB for 7.322e8 rows of 64 bytes = 69.05 B/row); the
+                # figure is per launch like `achieved`; null for other row sizes (not captured)
+                "traffic": int(69.05 * U_total) if M > 32 else None,
                 "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kernel_ms": round(scan_ms, 4),
                 "code_bytes_only_frac": round(M * U_total / (scan_ms * 1e-3) / 1e9 / peak, 4),
                 "share_of_step": round(scan_ms / ms_per_step, 4),
