@@ -24,12 +24,14 @@ struct fann_index {
     uint32_t scan_ring = 3;                // scan kernel: stages of the per-warp code-row ring, 0 = rows through registers (FANN_SCAN_RING)
     bool partition = true;                 // split lists into their dedup classes first (FANN_PARTITION=0: filter per pass)
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
+    uint32_t dedup_smem_half = 0;          // same for two CTAs per SM
+    uint32_t dedup_threads = 0;            // 0: chosen per call (geometry()); 1024 or 512: forced (FANN_DEDUP_THREADS)
     uint64_t launches = 0;
     // second stream + events for the dedup/scan overlap
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_dedup_done[kMaxChunks] = {}, ev_join = nullptr;
     // geometry of the last launches (fann_get_info)
-    uint32_t last_dedup_ctas = 0, last_scan_ctas = 0, last_scan_smem = 0, last_cap = 0, last_slots = 0, last_chunks = 0;
+    uint32_t last_dedup_threads = 1024, last_dedup_smem = 0, last_dedup_ctas = 0, last_scan_ctas = 0, last_scan_smem = 0, last_cap = 0, last_slots = 0, last_chunks = 0;
     // optional per-kernel timing
     bool timing = false;
     cudaEvent_t ev_lut[2] = {}, ev_plan[2] = {}, ev_dedup[kMaxChunks][2] = {}, ev_scan[kMaxChunks][2] = {};
@@ -68,15 +70,25 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // ---------------------------------------------------------------- geometry + workspace layout
 
 struct Geom {
-    uint32_t nslots_max, cap_c, dedup_smem;          // dedup: table slots per CTA, candidates per partition
+    uint32_t nslots_max, cap_c, dedup_smem, dedup_threads;   // dedup: table slots per CTA, candidates per partition, CTA shape
     uint32_t cap, scan_smem, ring;                   // scan: candidate-buffer keys, shared memory per CTA, ring depth
 };
 
-static void geometry(const fann_index *ix, uint32_t k, Geom *g)
+// Dedup CTA shape: one 1024-thread CTA per SM with the whole shared memory as its table, or -- when the mean candidate
+// list needs two or more partitions anyway -- two 512-thread CTAs per SM with half the table each, so that one computes
+// while the other waits at a barrier (partition_kernel makes the number of partitions free: each ID is read once).
+static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t total_cands, Geom *g)
 {
-    g->dedup_smem = ix->dedup_smem;
-    g->nslots_max = ((g->dedup_smem - kDedupTableOff) / 4) & ~3u;
+    g->dedup_threads = 1024; g->dedup_smem = ix->dedup_smem;
+    g->nslots_max = ((g->dedup_smem - dedup_table_off(1024)) / 4) & ~3u;
     g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
+    const uint64_t mean_c = total_cands / (B ? B : 1);
+    const bool split = ix->dedup_threads == 512 || (ix->dedup_threads == 0 && ix->partition && mean_c > g->cap_c);
+    if (split && ix->dedup_smem_half >= 32768) {
+        g->dedup_threads = 512; g->dedup_smem = ix->dedup_smem_half;
+        g->nslots_max = ((g->dedup_smem - dedup_table_off(512)) / 4) & ~3u;
+        g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);
+    }
     g->ring = ix->scan_ring;
     g->cap = (k <= 256 || g->ring) ? 4096u : 8192u;            // the ring takes the shared memory of the larger buffer
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap, g->ring);
@@ -134,7 +146,8 @@ extern "C" int fann_create(fann_index **out, int device)
     if (scan_max > smem_optin)
         return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
                     smem_optin, scan_max);
-    CUDA_TRY(cudaFuncSetAttribute(dedup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
+    CUDA_TRY(cudaFuncSetAttribute(dedup_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
+    CUDA_TRY(cudaFuncSetAttribute(dedup_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
     const int ring_max = (int)scan_smem_bytes(4096, 3);
     if (ring_max > smem_optin)
         return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
@@ -156,6 +169,12 @@ extern "C" int fann_create(fann_index **out, int device)
         int v = atoi(s);
         if (v == 32 || v == 64 || v == 128) CUDA_TRY(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)v));
     }
+    {   // two dedup CTAs per SM: each gets half of the SM's shared memory less the 1 KB the driver reserves per CTA
+        int per_sm = 0;
+        CUDA_TRY(cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device));
+        ix->dedup_smem_half = (uint32_t)((per_sm / 2 - 1024) & ~255);
+    }
+    if (const char *s = getenv("FANN_DEDUP_THREADS")) { int v = atoi(s); if (v == 512 || v == 1024) ix->dedup_threads = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_SMEM_KB")) {
         int v = atoi(s) * 1024;
         if (v >= 16 * 1024 && v <= smem_optin) ix->dedup_smem = (uint32_t)v;
@@ -191,8 +210,8 @@ extern "C" int fann_get_info(const fann_index *ix, fann_info *out)
     if (!ix || !out) return fail(FANN_EINVAL, "fann_get_info: NULL argument");
     out->N = ix->N; out->M = ix->M; out->row_bytes = ix->row_bytes;
     out->num_sms = (uint32_t)ix->num_sms;
-    out->dedup_threads = kDedupThreads; out->dedup_ctas = ix->last_dedup_ctas;
-    out->dedup_smem_bytes = ix->dedup_smem; out->table_slots = ix->last_slots;
+    out->dedup_threads = ix->last_dedup_threads; out->dedup_ctas = ix->last_dedup_ctas;
+    out->dedup_smem_bytes = ix->last_dedup_smem; out->table_slots = ix->last_slots;
     out->scan_threads = kScanThreads; out->scan_ctas = ix->last_scan_ctas;
     out->scan_smem_bytes = ix->last_scan_smem; out->scan_buffer_keys = ix->last_cap;
     out->chunks = ix->last_chunks;
@@ -297,7 +316,7 @@ extern "C" size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_
     if (!ix || !ix->codes) { fail(FANN_EINVAL, "fann_workspace_bytes: index has no codes"); return 0; }
     if (B == 0 || k == 0 || k > FANN_MAX_K) { fail(FANN_EINVAL, "fann_workspace_bytes: B=%u k=%u", B, k); return 0; }
     Geom g;
-    geometry(ix, k, &g);
+    geometry(ix, k, B, total_cands, &g);
     WsLayout w;
     ws_layout(B, total_cands, g, true, &w);
     return w.total;
@@ -343,7 +362,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     void *workspace, size_t workspace_bytes, cudaStream_t stream)
 {
     Geom g;
-    geometry(ix, k, &g);
+    geometry(ix, k, B, total_cands, &g);
     WsLayout w;
     ws_layout(B, total_cands, g, !dump, &w);
     if (!workspace || ((uintptr_t)workspace & 255) != 0)
@@ -405,13 +424,15 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
         dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
         if (timing && c > 0) cudaEventRecord(ix->ev_dedup[c][0], dstream);
-        dedup_kernel<<<ix->num_sms, kDedupThreads, g.dedup_smem, dstream>>>(dp);
+        if (g.dedup_threads == 512) dedup_kernel<512><<<2 * ix->num_sms, 512, g.dedup_smem, dstream>>>(dp);
+        else dedup_kernel<1024><<<ix->num_sms, 1024, g.dedup_smem, dstream>>>(dp);
         if (timing) cudaEventRecord(ix->ev_dedup[c][1], dstream);
         ix->launches++;
         CUDA_TRY(cudaGetLastError());
         if (overlap) CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], dstream));
     }
-    ix->last_dedup_ctas = (uint32_t)ix->num_sms; ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
+    ix->last_dedup_threads = g.dedup_threads; ix->last_dedup_smem = g.dedup_smem;
+    ix->last_dedup_ctas = (uint32_t)ix->num_sms * (g.dedup_threads == 512 ? 2u : 1u); ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
     ix->timed_chunks = timing ? chunks : 0; ix->timed_scan = false;
     if (!dump) {
         for (uint32_t c = 0; c < chunks; ++c) {
@@ -491,7 +512,7 @@ static void host_scratch_layout(const fann_index *ix, uint32_t B, uint32_t dsub,
                                 uint32_t k, HostScratch *h)
 {
     Geom g;
-    geometry(ix, k, &g);
+    geometry(ix, k, B, total_cands, &g);
     WsLayout w;
     ws_layout(B, total_cands, g, true, &w);
     size_t o = 0;

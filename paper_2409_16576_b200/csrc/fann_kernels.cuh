@@ -384,7 +384,7 @@ __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, ui
 }
 
 constexpr int kDedupIdsPerThread = 8;                // IDs a thread holds per batch (two 16-byte loads)
-constexpr uint32_t kDedupTableOff = 256 + 2 * kDedupThreads * 4;   // bookkeeping + two retry queues precede the table
+__host__ __device__ constexpr uint32_t dedup_table_off(uint32_t threads) { return 256 + 2 * threads * 4; }   // bookkeeping + two retry queues precede the table
 
 // PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel takes
 // a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-memory
@@ -399,14 +399,17 @@ constexpr uint32_t kDedupTableOff = 256 + 2 * kDedupThreads * 4;   // bookkeepin
 // one slot ends up holding it.  Each CTA pass handles the IDs of one query that fall into one partition
 // (an ID range in ordered mode, a hash class in hashed mode), 8 per thread per batch, then compacts its
 // table in slot order into the query's distinct list.
-__global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupParams p)
+// T threads per CTA: 1024 (one CTA per SM, the whole shared memory as one table) or 512 (two CTAs per SM with half
+// the table each: one computes while the other waits at a barrier).
+template <int T>
+__global__ void __launch_bounds__(T, T == 1024 ? 1 : 2) dedup_kernel(const DedupParams p)
 {
     constexpr int R = kDedupIdsPerThread;
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base [2,3] queue lengths [4] kEmpty [32..63] warp counts
     uint32_t *wsum = misc + 32, *qcnt = misc + 2;
-    uint32_t *queue = reinterpret_cast<uint32_t *>(smem + 256);              // two retry queues of kDedupThreads IDs
-    uint32_t *table = reinterpret_cast<uint32_t *>(smem + kDedupTableOff);
+    uint32_t *queue = reinterpret_cast<uint32_t *>(smem + 256);              // two retry queues of T IDs
+    uint32_t *table = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T));
     const uint32_t tbl = (uint32_t)__cvta_generic_to_shared(table);
     const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 4);   // a word that always holds kEmpty
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -449,7 +452,7 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
         {
             uint4 *t4 = reinterpret_cast<uint4 *>(table);
             const uint4 e4 = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
-            for (uint32_t i = tid; i < (nslots >> 2); i += kDedupThreads) t4[i] = e4;
+            for (uint32_t i = tid; i < (nslots >> 2); i += T) t4[i] = e4;
         }
 
         // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list.
@@ -474,7 +477,7 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
             return tbl + (__umulhi(a, nslots) << 2);
         };
         const uint32_t tbl_end = tbl + (nslots << 2);
-        uint4 nxt0 = load_vec(tid), nxt1 = load_vec(tid + kDedupThreads);   // this thread's vectors of the next batch
+        uint4 nxt0 = load_vec(tid), nxt1 = load_vec(tid + T);   // this thread's vectors of the next batch
         if (tid == 0) { qcnt[0] = 0; qcnt[1] = 0; }
         __syncthreads();                                       // table cleared, queues empty
 
@@ -484,11 +487,11 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
         // at `none_addr`, a word that always holds kEmpty == kIdNone: it "finds itself" there, so probe and
         // verify need no special case and no predicated loads.
         uint32_t qin = 0, qn = 0;                              // queue read by this batch, its length
-        for (uint32_t vbase = 0; vbase < nvec || qn; vbase += 2 * kDedupThreads) {
+        for (uint32_t vbase = 0; vbase < nvec || qn; vbase += 2 * T) {
             uint32_t id[R + 1] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w, kIdNone};
             uint32_t sa[R + 1];
-            nxt0 = load_vec(vbase + 2 * kDedupThreads + tid);
-            nxt1 = load_vec(vbase + 3 * kDedupThreads + tid);
+            nxt0 = load_vec(vbase + 2 * T + tid);
+            nxt1 = load_vec(vbase + 3 * T + tid);
             if (!hashed) {
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
@@ -510,8 +513,8 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                 }
             }
             sa[R] = none_addr;
-            if (tid < qn) { id[R] = queue[qin * kDedupThreads + tid]; sa[R] = place(id[R]); }
-            uint32_t *qpush = queue + (qin ^ 1u) * kDedupThreads;
+            if (tid < qn) { id[R] = queue[qin * T + tid]; sa[R] = place(id[R]); }
+            uint32_t *qpush = queue + (qin ^ 1u) * T;
             for (;;) {
                 // probe (reads only): to the ID itself (a repeat) or to the first empty slot
                 uint32_t cur[R + 1];
@@ -565,7 +568,7 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
                     for (int j = 0; j <= R; ++j) {
                         if (id[j] == kIdNone) continue;
                         const uint32_t pos = atomicAdd(&qcnt[qin ^ 1u], 1u);
-                        if (pos < (uint32_t)kDedupThreads) { qpush[pos] = id[j]; id[j] = kIdNone; sa[j] = none_addr; }
+                        if (pos < (uint32_t)T) { qpush[pos] = id[j]; id[j] = kIdNone; sa[j] = none_addr; }
                     }
                     all = id[0];
 #pragma unroll
@@ -575,14 +578,14 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
             }
             qin ^= 1u;                                         // the queue just filled is the next batch's input
             qn = qcnt[qin];
-            if (qn > (uint32_t)kDedupThreads) qn = kDedupThreads;
+            if (qn > (uint32_t)T) qn = T;
         }
 
         // compact the table in slot order: count per warp range, scan, write
         {
             const uint4 *t4 = reinterpret_cast<const uint4 *>(table);
             const uint32_t n4 = nslots >> 2;
-            const uint32_t chunk = ((n4 + kDedupThreads - 1) / kDedupThreads) * 32;   // vectors per warp, multiple of 32
+            const uint32_t chunk = ((n4 + T - 1) / T) * 32;   // vectors per warp, multiple of 32
             const uint32_t v0 = warp * chunk < n4 ? warp * chunk : n4;
             const uint32_t v1 = v0 + chunk < n4 ? v0 + chunk : n4;
             uint32_t c = 0;
@@ -593,6 +596,7 @@ __global__ void __launch_bounds__(kDedupThreads, 1) dedup_kernel(const DedupPara
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
             if (lane == 0) wsum[warp] = c;
+            if (T < 1024 && tid >= T / 32 && tid < 32) wsum[tid] = 0;   // warps that do not exist
             __syncthreads();
             if (warp == 0) {
                 const uint32_t wv = wsum[lane];

@@ -133,8 +133,8 @@ def test_lut_query_on_centroid_is_exact_zero(fann, tiny):
 # ------------------------------------------------------------------ (5) dedup
 
 def _dedup_check(fann, w, off, ids, ascending=None):
-    """ascending: query indices whose distinct list must come out in ascending order (one partition,
-    ordered placement) up to the shuffle inside a compaction step and the few IDs displaced by probing."""
+    """ascending: query indices whose distinct list must come out in ascending order (ordered placement),
+    up to the shuffle inside a compaction step, the few IDs displaced by probing and the partition seams."""
     ix = fann.FannIndex(0)
     ix.load_codes(w.codes.to(DEV))
     o = torch.from_numpy(np.ascontiguousarray(off, dtype=np.int64)).to(DEV)
@@ -150,7 +150,8 @@ def _dedup_check(fann, w, off, ids, ascending=None):
         if ascending and b in ascending and got.size > 1:
             g64 = got.astype(np.int64)                         # ascending beyond the 128-slot compaction step
             far = np.count_nonzero(g64[512:] < g64[:-512])
-            assert far <= 0.01 * got.size, f"query {b}: {far} of {got.size} ids descend over a distance of 512"
+            # each partition of the query (at most 8) contributes one ascending segment, in any order
+            assert far <= 0.01 * got.size + 8 * 512, f"query {b}: {far} of {got.size} ids descend over a distance of 512"
 
 
 def test_dedup_sets_bit_exact(fann, tiny_local, w_int, w_k1000):
