@@ -432,7 +432,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         if (overlap) CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], dstream));
     }
     ix->last_dedup_threads = g.dedup_threads; ix->last_dedup_smem = g.dedup_smem;
-    ix->last_dedup_ctas = (uint32_t)ix->num_sms * (g.dedup_threads == 512 ? 2u : 1u); ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
+    ix->last_dedup_ctas = (uint32_t)ix->num_sms * (1024u / g.dedup_threads); ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
     ix->timed_chunks = timing ? chunks : 0; ix->timed_scan = false;
     if (!dump) {
         for (uint32_t c = 0; c < chunks; ++c) {

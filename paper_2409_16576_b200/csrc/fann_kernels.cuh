@@ -297,7 +297,7 @@ __device__ __forceinline__ uint32_t hash_round1(uint32_t x) { return (x ^ (x >> 
 
 __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, uint32_t C);
 
-constexpr uint32_t kMaxPartBuckets = 8;              // partition_kernel handles 2..8 classes per query
+constexpr uint32_t kMaxPartBuckets = 16;             // partition_kernel handles 2..16 classes per query
 constexpr int kPartThreads = 512;
 
 struct PartParams {
@@ -402,7 +402,7 @@ __host__ __device__ constexpr uint32_t dedup_table_off(uint32_t threads) { retur
 // T threads per CTA: 1024 (one CTA per SM, the whole shared memory as one table) or 512 (two CTAs per SM with half
 // the table each: one computes while the other waits at a barrier).
 template <int T>
-__global__ void __launch_bounds__(T, T == 1024 ? 1 : 2) dedup_kernel(const DedupParams p)
+__global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
 {
     constexpr int R = kDedupIdsPerThread;
     extern __shared__ __align__(16) unsigned char smem[];
