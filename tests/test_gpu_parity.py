@@ -171,6 +171,8 @@ def test_dedup_adversarial(fann, tiny_local):
         np.array([N, N + 1, 2 ** 31, NONE - 1, 5], dtype=np.uint32),            # out of range except one
         rng.integers(0, 50, size=40_000).astype(np.uint32),                     # 50 ids, long list
         np.concatenate([rng.permutation(N)[:60_000].astype(np.uint32)] * 2),    # 120k, each twice
+        rng.permutation(N)[:41_500].astype(np.uint32),      # no repeat, fills one table to 74 %: many store races
+        rng.permutation(N)[:20_900].astype(np.uint32),      # the same for the two-CTA shape's half table
     ]
     off = np.zeros(len(lists) + 1, dtype=np.int64)
     off[1:] = np.cumsum([len(x) for x in lists])
