@@ -157,6 +157,9 @@ int fann_workspace_status(fann_index *ix, const void *workspace, void *stream);
  * copies queries / candidate lists host->device into `device_scratch`, runs
  * fann_build_lut + fann_dedup_scan_topk, copies ids/dists/counts back and
  * synchronises `stream` before returning.  Codebooks stay on the device.
+ * From 16 MB of candidate IDs up, the IDs go up in 8 chunks of queries on a
+ * stream of the index's own and the path runs chunk by chunk behind them
+ * (queries are independent), so the transfer and the kernels overlap.
  * queries_h, cand_offsets_h, cand_ids_h, out_*_h: host pointers (pinned memory
  * gives asynchronous copies); layouts as above.  out_counts_h may be NULL.
  * device_scratch: device, >= fann_search_host_scratch_bytes(...), 256-byte aligned.

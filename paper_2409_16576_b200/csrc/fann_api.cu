@@ -77,13 +77,14 @@ struct Geom {
 // Dedup CTA shape: one 1024-thread CTA per SM with the whole shared memory as its table, or -- when the mean candidate
 // list needs two or more partitions anyway -- two 512-thread CTAs per SM with half the table each, so that one computes
 // while the other waits at a barrier (partition_kernel makes the number of partitions free: each ID is read once).
-static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t total_cands, Geom *g)
+static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t total_cands, Geom *g, uint32_t shape = 0)
 {
     g->dedup_threads = 1024; g->dedup_smem = ix->dedup_smem;
     g->nslots_max = ((g->dedup_smem - dedup_table_off(1024)) / 4) & ~3u;
     g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
     const uint64_t mean_c = total_cands / (B ? B : 1);
-    const bool split = ix->dedup_threads == 512 || (ix->dedup_threads == 0 && ix->partition && mean_c > g->cap_c);
+    const bool split = shape ? shape == 512
+                             : (ix->dedup_threads == 512 || (ix->dedup_threads == 0 && ix->partition && mean_c > g->cap_c));
     if (split && ix->dedup_smem_half >= 32768) {
         g->dedup_threads = 512; g->dedup_smem = ix->dedup_smem_half;
         g->nslots_max = ((g->dedup_smem - dedup_table_off(512)) / 4) & ~3u;
@@ -359,10 +360,11 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     const int64_t *cand_offsets, const uint32_t *cand_ids, uint64_t total_cands,
                     uint32_t k, uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
                     uint32_t *out_uniq, uint32_t *uniq_ids, uint32_t *uniq_counts,
-                    void *workspace, size_t workspace_bytes, cudaStream_t stream)
+                    void *workspace, size_t workspace_bytes, cudaStream_t stream,
+                    uint32_t shape = 0, bool keep_status = false)
 {
     Geom g;
-    geometry(ix, k, B, total_cands, &g);
+    geometry(ix, k, B, total_cands, &g, shape);
     WsLayout w;
     ws_layout(B, total_cands, g, !dump, &w);
     if (!workspace || ((uintptr_t)workspace & 255) != 0)
@@ -381,7 +383,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     const bool timing = ix->timing;
     if (timing) cudaEventRecord(ix->ev_plan[0], stream);
     plan_kernel<<<1, 1024, 0, stream>>>((const long long *)cand_offsets, B, g.cap_c, w.max_items, hdr, S,
-                                        item_start, items, uniq_counts);
+                                        item_start, items, uniq_counts, keep_status ? 1u : 0u);
     mode_kernel<<<(B + 7) / 8, 256, 0, stream>>>((const long long *)cand_offsets, cand_ids, B, ix->N,
                                                   ix->force_mode, mode);
     if (timing) cudaEventRecord(ix->ev_plan[1], stream);
@@ -562,15 +564,30 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
     char *s = (char *)device_scratch;
     CUDA_TRY(cudaMemcpyAsync(s + h.queries, queries_h, (size_t)B * ix->M * dsub * 4, cudaMemcpyHostToDevice, stream));
     CUDA_TRY(cudaMemcpyAsync(s + h.offsets, cand_offsets_h, ((size_t)B + 1) * 8, cudaMemcpyHostToDevice, stream));
-    if (total)
-        CUDA_TRY(cudaMemcpyAsync(s + h.ids, cand_ids_h, (size_t)total * 4, cudaMemcpyHostToDevice, stream));
     int rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
     if (rc != FANN_OK) return rc;
-    rc = fann_dedup_scan_topk(ix, (const float *)(s + h.lut), B, (const int64_t *)(s + h.offsets),
-                              (const uint32_t *)(s + h.ids), total, k, (uint32_t *)(s + h.out_ids),
-                              (float *)(s + h.out_dists), (uint32_t *)(s + h.out_counts), nullptr,
-                              s + h.ws, h.ws_bytes, stream);
-    if (rc != FANN_OK) return rc;
+    // The candidate IDs are the bulk of the transfer (PAPER.md:L125 step (4)).  They go up in chunks of queries
+    // on the index's side stream, and the path runs chunk by chunk behind them: queries are independent, and
+    // offsets stay absolute, so a chunk is the same call on a sub-range of the batch.
+    Geom g;
+    geometry(ix, k, B, total, &g);                             // one dedup CTA shape for all chunks: the layout depends on it
+    const uint32_t nchunk = (B >= 64 && total >= (4u << 20) && ix->chunks == 1) ? 8u : 1u;   // 16 MB of IDs and up
+    CUDA_TRY(cudaEventRecord(ix->ev_fork, stream));
+    CUDA_TRY(cudaStreamWaitEvent(ix->side, ix->ev_fork, 0));   // the scratch may still be in use by earlier work on `stream`
+    for (uint32_t c = 0; c < nchunk; ++c) {
+        const uint32_t b0 = (uint32_t)((uint64_t)B * c / nchunk), b1 = (uint32_t)((uint64_t)B * (c + 1) / nchunk);
+        const uint64_t e0 = (uint64_t)cand_offsets_h[b0], e1 = (uint64_t)cand_offsets_h[b1];
+        if (e1 > e0)
+            CUDA_TRY(cudaMemcpyAsync(s + h.ids + e0 * 4, cand_ids_h + e0, (size_t)(e1 - e0) * 4, cudaMemcpyHostToDevice, ix->side));
+        CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], ix->side));
+        CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_dedup_done[c], 0));
+        rc = run_path(ix, false, (const float *)(s + h.lut) + (size_t)b0 * ix->M * 256, b1 - b0,
+                      (const int64_t *)(s + h.offsets) + b0, (const uint32_t *)(s + h.ids), total, k,
+                      (uint32_t *)(s + h.out_ids) + (size_t)b0 * k, (float *)(s + h.out_dists) + (size_t)b0 * k,
+                      (uint32_t *)(s + h.out_counts) + b0, nullptr, nullptr, nullptr,
+                      s + h.ws, h.ws_bytes, stream, g.dedup_threads, c > 0);
+        if (rc != FANN_OK) return rc;
+    }
     CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
     CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
     if (out_counts_h)

@@ -146,7 +146,7 @@ __global__ void build_lut_kernel(const float *__restrict__ queries, const float 
 // per-query distinct counts and the work counters.
 __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t B, uint32_t cap_c,
                             uint32_t max_items, WsHeader *hdr, uint32_t *S, uint32_t *item_start,
-                            uint2 *items, uint32_t *uniq_counts)
+                            uint2 *items, uint32_t *uniq_counts, uint32_t keep_status)
 {
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t running;
@@ -195,7 +195,8 @@ __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t
         const bool over = running > max_items;
         item_start[B] = over ? 0u : running;
         if (over) for (uint32_t b = 0; b < B; ++b) item_start[b] = 0;   // no dedup work; scan sees U = 0
-        hdr->status = over ? kStatusPlanOverflow : 0u;
+        // a later chunk of the same batch (fann_search_host) keeps what the earlier chunks reported
+        hdr->status = (keep_status ? hdr->status : 0u) | (over ? kStatusPlanOverflow : 0u);
         hdr->n_items = over ? 0u : running;
     }
 }

@@ -304,6 +304,67 @@ def test_host_entry_matches_device_entry(fann, w_i8):
     assert np.array_equal(od.numpy(), res[1]) and np.array_equal(oc.numpy().view(np.uint32), res[2])
 
 
+def test_host_entry_in_chunks_matches_device_entry_and_oracle(fann):
+    """A batch large enough (> 4 M candidate IDs) for fann_search_host to send the IDs up in 8 chunks of
+    queries behind which the path runs chunk by chunk: same bytes as the one-call device path, and the
+    first queries equal the oracle."""
+    w = make_workload(mini("u8_10m_m32", N=1_000_000, n_lists=2_000, B=160, codes_mode="histogram"))
+    assert w.cand_ids.numel() > (4 << 20)
+    ix, _, res = gpu_search(fann, w)
+    B, k, total = w.cfg.B, w.cfg.k, w.cand_ids.numel()
+    need = fann.fann_search_host_scratch_bytes(ix.handle, B, w.cfg.dsub, total, k)
+    scratch = torch.empty(need, dtype=torch.uint8, device=DEV)
+    q_h, off_h, ids_h = w.queries.pin_memory(), w.cand_offsets.pin_memory(), w.cand_ids.pin_memory()
+    oi = torch.empty((B, k), dtype=torch.int32).pin_memory()
+    od = torch.empty((B, k), dtype=torch.float32).pin_memory()
+    oc = torch.empty(B, dtype=torch.int32).pin_memory()
+    for _ in range(2):                                        # twice: the scratch is reused across batches
+        oi.fill_(0)
+        fann.fann_search_host(ix.handle, q_h, B, w.codebooks.to(DEV), w.cfg.dsub, off_h, ids_h, k, oi, od, oc,
+                              scratch, need, torch.cuda.current_stream().cuda_stream)
+        assert np.array_equal(oi.numpy().view(np.uint32), res[0])
+        assert np.array_equal(od.numpy(), res[1]) and np.array_equal(oc.numpy().view(np.uint32), res[2])
+    nq = 12
+    off = w.cand_offsets.numpy()[: nq + 1]
+    ref = oracle.search(w.queries.numpy()[:nq], w.codebooks.numpy(), w.codes.numpy(), off,
+                        w.cand_ids.numpy().view(np.uint32)[: off[-1]], k)
+    assert np.array_equal(oi.numpy().view(np.uint32)[:nq], ref["ids"]) and np.array_equal(od.numpy()[:nq], ref["dists"])
+
+
+@pytest.mark.parametrize("name,nq", [("u8_10m_m32", 48), ("u8_1b_m64", 12)])
+def test_full_size_configs_sampled_against_oracle(fann, name, nq):
+    """BASELINE's configs at full size, in the launch configuration bench.py times (same calls, same
+    workspace sizing): the first nq queries are compared with the oracle byte for byte (integer-exact
+    regime), and every query with properties that hold at any size."""
+    import bench
+    cfg = CONFIGS[name]
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 2 * cfg.N * cfg.M + (40 << 30):              # workload's codes + the library's copy + per-batch arrays
+        pytest.skip("not enough free device memory for this config")
+    w = make_workload(cfg, device=DEV)
+    B, k = cfg.B, cfg.k
+    ix = fann.FannIndex(0)
+    ix.load_codes(w.codes)
+    lut = ix.build_lut(w.queries, w.codebooks)
+    o = ix.dedup_scan_topk(lut, w.cand_offsets, w.cand_ids, k, check=True)
+    torch.cuda.synchronize()
+    ids, dists, counts, uniq = o
+    # any size: counts = min(k, U), U <= C, distances ascending, no ID twice in a row of results
+    C = (w.cand_offsets[1:] - w.cand_offsets[:-1])
+    assert bool((uniq.long() <= C).all()) and bool((counts.long() == torch.clamp(uniq.long(), max=k)).all())
+    assert bool((dists[:, 1:] >= dists[:, :-1]).all())
+    srt = torch.sort(ids.long() & 0xFFFFFFFF, dim=1).values
+    assert bool(((srt[:, 1:] != srt[:, :-1]) | (srt[:, 1:] == 0xFFFFFFFF)).all())
+    # sampled: byte equality with the oracle on the first nq queries
+    _, r, _ = bench.oracle_sample(w, nq, w.codes)
+    assert np.array_equal(np_u32(uniq[:nq]), r["uniq"])
+    assert np.array_equal(np_u32(ids[:nq]), r["ids"]) and np.array_equal(dists[:nq].cpu().numpy(), r["dists"])
+    ix.close()
+    del w, lut, o
+    torch.cuda.empty_cache()
+
+
 def test_load_codes_from_host_and_in_chunks(fann, w_i8):
     w = w_i8
     ix = fann.FannIndex(0)
