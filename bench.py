@@ -242,7 +242,7 @@ def main():
     roofline = {"bound": "hbm", "kernel": "scan_kernel", "achieved": round(achieved, 1), "peak": peak,
                 "unit": "GB/s", "frac": round(achieved / peak, 4),
                 # dram__bytes_read+write of this kernel per gathered row, measured by ncu on this very workload
-                # (profiles/r1j_launches_u8_1b_m64.md: 50.56 GB for 7.322e8 rows of 64 bytes = 69.05 B/row); the
+                # (profiles/r1k_launches_u8_1b_m64.md: 50.56 GB for 7.322e8 rows of 64 bytes = 69.05 B/row); the
                 # figure is per launch like `achieved`; null for other row sizes (not captured)
                 "traffic": int(69.05 * U_total) if M > 32 else None,
                 "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kernel_ms": round(scan_ms, 4),
