@@ -99,8 +99,9 @@ int fann_build_lut(fann_index *ix, const float *queries, uint32_t B,
  * Bytes of device workspace fann_dedup_scan_topk / fann_dedup_only need for a
  * batch of B queries holding total_cands candidate IDs in all.  The workspace
  * is the paper's per-query working memory turned inside out:
- * the caller allocates it once and reuses it across batches.  Returns 0 on a
- * bad argument (see fann_last_error).
+ * the caller allocates it once and reuses it across batches.  About 12 bytes per
+ * candidate ID (the distinct IDs, and the candidate lists split into dedup classes)
+ * plus small per-query arrays.  Returns 0 on a bad argument (see fann_last_error).
  */
 size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t total_cands, uint32_t k);
 
@@ -178,13 +179,13 @@ typedef struct fann_info {
     uint32_t M;                /* PQ bytes per vector                                         */
     uint32_t row_bytes;        /* stored row stride: 16, 32 or 64                             */
     uint32_t num_sms;          /* multiprocessors of the device                               */
-    uint32_t dedup_threads;    /* threads per CTA of the dedup kernel                         */
-    uint32_t dedup_ctas;       /* persistent CTAs of the last dedup launch                    */
+    uint32_t dedup_threads;    /* threads per CTA of the last dedup launch: 1024 or 512       */
+    uint32_t dedup_ctas;       /* persistent CTAs of the last dedup launch (1 or 2 per SM)    */
     uint32_t dedup_smem_bytes; /* dynamic shared memory per dedup CTA                         */
-    uint32_t table_slots;      /* dedup hash-table slots one CTA can hold                     */
+    uint32_t table_slots;      /* dedup table slots one CTA can hold                          */
     uint32_t scan_threads;     /* threads per CTA of the scan kernel                          */
     uint32_t scan_ctas;        /* persistent CTAs of the last scan launch                     */
-    uint32_t scan_smem_bytes;  /* dynamic shared memory per scan CTA                          */
+    uint32_t scan_smem_bytes;  /* dynamic shared memory per scan CTA (table, buffer, ring)    */
     uint32_t scan_buffer_keys; /* top-k candidate buffer of a scan CTA, in (dist, id) keys    */
     uint32_t chunks;           /* batch chunks of the last call (dedup i+1 beside scan i)     */
     uint32_t reserved;

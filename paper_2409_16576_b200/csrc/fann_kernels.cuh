@@ -3,13 +3,17 @@
 // Kernels (section 3, steps (1)(5)(6)(7)):
 //   repack_rows_kernel   fann_load_codes: pad rows of M bytes to 16 / 32 / 64 bytes
 //   build_lut_kernel     (1) lut[b][m][j] = sum_t (q - c)^2
-//   plan_kernel          split each query into S_b hash partitions that fit one SM's table
+//   plan_kernel          S_b partitions per query so that each fits one CTA's dedup table; work-item list
 //   mode_kernel          per query: order-preserving or hashed placement in the dedup table
-//   dedup_kernel         (5) shared-memory dedup table, one (query, partition) per CTA pass;
-//                        writes the distinct IDs of every query as a compact list, ascending
-//                        (up to probe displacement) in ordered mode
-//   scan_kernel          (6) code-row gather + Eq. 1 ADC  (7) streaming top-k, one query per
-//                        CTA pass; writes out_ids / out_dists / counts
+//   partition_kernel     split each query's candidate IDs into its S_b classes (ID ranges or hash
+//                        classes), so that each dedup pass reads only its own IDs
+//   dedup_kernel<T>      (5) shared-memory dedup table, one (query, partition) per CTA pass; probe /
+//                        store / verify phases separated by barriers, no atomics in the table;
+//                        writes the distinct IDs of every query as a compact list, ascending in
+//                        ordered mode (up to the compaction step and probe displacement)
+//   scan_kernel<G,NB,D>  (6) code-row gather through a per-warp shared-memory ring filled by
+//                        asynchronous copies + Eq. 1 ADC from a conflict-free table  (7) streaming
+//                        top-k, one query per CTA pass; writes out_ids / out_dists / counts
 //   gather_probe_kernel  measurement only: the scan kernel's row gather without its arithmetic
 #pragma once
 #include <cuda_runtime.h>
