@@ -230,6 +230,26 @@ def test_k1000_partitions_bytes(fann, w_k1000):
     assert ties > 0
 
 
+@pytest.mark.parametrize("env", [
+    {"FANN_DEDUP_THREADS": "512"},                       # two dedup CTAs per SM, half tables
+    {"FANN_DEDUP_THREADS": "1024"},                      # one dedup CTA per SM
+    {"FANN_PARTITION": "0"},                             # dedup passes filter the whole list themselves
+    {"FANN_DEDUP_MODE": "1"},                            # hashed placement and hash classes
+    {"FANN_DEDUP_MODE": "1", "FANN_PARTITION": "0"},
+    {"FANN_SCAN_RING": "0"},                             # code rows through registers
+])
+def test_every_code_path_gives_the_same_bytes(fann, w_k1000, w_i8, monkeypatch, env):
+    """The library picks CTA shapes, placement and staging by itself; each alternative (also the
+    fallbacks it takes on bunched IDs or refused splits) must give the oracle's bytes."""
+    for key in ("FANN_DEDUP_THREADS", "FANN_PARTITION", "FANN_DEDUP_MODE", "FANN_SCAN_RING"):
+        monkeypatch.delenv(key, raising=False)
+    for key, val in env.items():
+        monkeypatch.setenv(key, val)
+    for w in (w_k1000, w_i8):
+        _, _, res = gpu_search(fann, w)
+        check_exact(res, orc_search(w))
+
+
 def test_fp32_config_band(fann, w_f32):
     _, _, res = gpu_search(fann, w_f32)
     band_all(w_f32, res)
