@@ -121,7 +121,7 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
 // ---------------------------------------------------------------- lifecycle
 
 extern "C" const char *fann_last_error(void) { return g_err; }
-extern "C" const char *fann_version(void) { return "fann 0.2 sm_100a"; }
+extern "C" const char *fann_version(void) { return "fann 0.3 sm_100a"; }
 
 template <int G, int NB, int D>
 static cudaError_t set_scan_attr(int smem)
