@@ -301,9 +301,14 @@ extern "C" int fann_build_lut(fann_index *ix, const float *queries, uint32_t B,
     if (dsub == 0 || dsub > 64) return fail(FANN_EUNSUPPORTED, "fann_build_lut: dsub=%u not in 1..64", dsub);
     DeviceGuard guard(ix->device);
     cudaStream_t stream = (cudaStream_t)stream_;
-    const uint64_t units = (uint64_t)B * ix->M * 64;
+    const uint64_t blocks = (uint64_t)B * ((ix->M + 3) / 4);
+    if (blocks > 0x7FFFFFFFull) return fail(FANN_EUNSUPPORTED, "fann_build_lut: B=%u too large for one launch", B);
+    const bool vec = (((uintptr_t)codebooks | (uintptr_t)queries) & 15) == 0;   // float4 reads of the codebook
     if (ix->timing) cudaEventRecord(ix->ev_lut[0], stream);
-    build_lut_kernel<<<(unsigned)((units + 255) / 256), 256, 0, stream>>>(queries, codebooks, lut, B, ix->M, dsub);
+    if (vec && dsub == 2) build_lut_kernel<2><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
+    else if (vec && dsub == 4) build_lut_kernel<4><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
+    else if (vec && dsub == 8) build_lut_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
+    else build_lut_kernel<0><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
     if (ix->timing) { cudaEventRecord(ix->ev_lut[1], stream); ix->have_lut = true; }
     ix->launches++;
     CUDA_TRY(cudaGetLastError());

@@ -118,25 +118,47 @@ __global__ void repack_rows_kernel(const uint8_t *__restrict__ src, uint8_t *__r
 
 // ---------------------------------------------------------------- (1) lookup table
 
-// One thread = 4 consecutive centroids j of one (query, sub-space).
-__global__ void build_lut_kernel(const float *__restrict__ queries, const float *__restrict__ codebooks,
-                                 float *__restrict__ lut, uint32_t B, uint32_t M, uint32_t dsub)
+// One thread = 4 consecutive centroids j of one (query, sub-space); one block = 4 sub-spaces of one query.
+// DS = dsub when it is 2, 4 or 8 (the thread's 4 x dsub codebook floats are contiguous and 16-byte aligned:
+// read as float4), else 0 (any dsub, scalar loads).  Sum over t ascending with FMA in both.
+template <int DS>
+__global__ void __launch_bounds__(256) build_lut_kernel(const float *__restrict__ queries,
+                                                        const float *__restrict__ codebooks,
+                                                        float *__restrict__ lut, uint32_t M, uint32_t dsub_rt)
 {
-    uint64_t u = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t per_q = (uint64_t)M * 64;
-    if (u >= (uint64_t)B * per_q) return;
-    uint32_t b = (uint32_t)(u / per_q);
-    uint32_t rem = (uint32_t)(u % per_q);
-    uint32_t m = rem >> 6, j0 = (rem & 63) << 2;
-    const float *q = queries + (size_t)b * M * dsub + (size_t)m * dsub;
+    const uint32_t blocks_per_q = (M + 3) >> 2;
+    const uint32_t b = blockIdx.x / blocks_per_q;
+    const uint32_t m = ((blockIdx.x - b * blocks_per_q) << 2) + (threadIdx.x >> 6);
+    if (m >= M) return;
+    const uint32_t j0 = (threadIdx.x & 63u) << 2;
+    const uint32_t dsub = DS ? (uint32_t)DS : dsub_rt;
+    const float *q = queries + ((size_t)b * M + m) * dsub;
     const float *c = codebooks + ((size_t)m * 256 + j0) * dsub;
     float s[4] = {0.f, 0.f, 0.f, 0.f};
-    for (uint32_t t = 0; t < dsub; ++t) {
-        float qv = __ldg(q + t);
+    if constexpr (DS > 0) {
+        float cv[4 * DS], qv[DS];
 #pragma unroll
-        for (int jj = 0; jj < 4; ++jj) {
-            float dlt = qv - __ldg(c + jj * dsub + t);
-            s[jj] = fmaf(dlt, dlt, s[jj]);
+        for (int i = 0; i < DS; ++i) {
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(c) + i);
+            cv[4 * i] = v.x; cv[4 * i + 1] = v.y; cv[4 * i + 2] = v.z; cv[4 * i + 3] = v.w;
+        }
+#pragma unroll
+        for (int t = 0; t < DS; ++t) qv[t] = __ldg(q + t);
+#pragma unroll
+        for (int t = 0; t < DS; ++t)
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                const float dlt = qv[t] - cv[jj * DS + t];
+                s[jj] = fmaf(dlt, dlt, s[jj]);
+            }
+    } else {
+        for (uint32_t t = 0; t < dsub; ++t) {
+            const float qv = __ldg(q + t);
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                const float dlt = qv - __ldg(c + jj * dsub + t);
+                s[jj] = fmaf(dlt, dlt, s[jj]);
+            }
         }
     }
     *reinterpret_cast<float4 *>(lut + ((size_t)b * M + m) * 256 + j0) = make_float4(s[0], s[1], s[2], s[3]);

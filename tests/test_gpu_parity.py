@@ -120,6 +120,19 @@ def test_lut_integer_exact_and_fp32(fann, w_int, w_f32, w_i8):
             assert np.array_equal(lut.astype(np.float64), lut64)
 
 
+@pytest.mark.parametrize("M,dsub", [(5, 3), (7, 1), (16, 8), (25, 4), (3, 2), (64, 2), (6, 5)])
+def test_lut_any_shape(fann, M, dsub):
+    """Sub-space counts that do not fill a block of 4, and dsub with and without the float4 codebook path."""
+    rng = np.random.default_rng(M * 100 + dsub)
+    B = 37
+    q = torch.from_numpy(rng.normal(size=(B, M * dsub)).astype(np.float32))
+    cb = torch.from_numpy(rng.normal(size=(M, 256, dsub)).astype(np.float32))
+    ix = fann.FannIndex(0)
+    ix.load_codes(torch.zeros((8, M), dtype=torch.uint8, device=DEV))
+    lut = ix.build_lut(q.to(DEV), cb.to(DEV)).cpu().numpy()
+    check_lut(lut, oracle.build_lut(q.numpy(), cb.numpy()))
+
+
 def test_lut_query_on_centroid_is_exact_zero(fann, tiny):
     w = tiny
     q = w.queries.clone()
