@@ -664,6 +664,7 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
 //   [64, +2 KB)          prune sample keys        [.., +1 KB) their ranks
 //   [3136, +cap*8)       top-k candidate buffer, 64-bit keys (dist bits << 32 | id)
 //   [.., +64 KB)         lookup table of the query, c-major: entry (c, col) at byte c*256 + col*4
+//   [.., +warps*D*2.5 KB) per-warp rings of D stages (2 KB of code rows + the rows' IDs), D > 0 only
 constexpr uint32_t kScanBufOff = 64 + kSample * 8 + kSample * 4;
 constexpr uint32_t kRingStageBytes = 2048 + 512;     // 2 KB of code rows + the stage's IDs (32 .. 128 of them)
 __host__ __device__ inline size_t scan_smem_bytes(uint32_t cap, uint32_t ring_depth = 0)
@@ -1035,7 +1036,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 
 // ---------------------------------------------------------------- measurement: gather only
 
-// Load flavours the probe can compare (flavour 0 is what the scan kernel uses).
+// Load flavours the probe can compare (flavour 1 has the qualifiers of the scan kernel's copies).
 __device__ __forceinline__ uint4 probe_load16(const void *p, uint32_t flavor, uint64_t pol)
 {
     uint4 r;
