@@ -187,7 +187,7 @@ typedef struct fann_info {
     uint32_t scan_ctas;        /* persistent CTAs of the last scan launch                     */
     uint32_t scan_smem_bytes;  /* dynamic shared memory per scan CTA (table, buffer, ring)    */
     uint32_t scan_buffer_keys; /* top-k candidate buffer of a scan CTA, in (dist, id) keys    */
-    uint32_t chunks;           /* batch chunks of the last call (dedup i+1 beside scan i)     */
+    uint32_t chunks;           /* batch chunks of the last call (1 unless FANN_CHUNKS is set) */
     uint32_t reserved;
     uint64_t kernel_launches;  /* kernels this index has launched so far                      */
 } fann_info;
@@ -200,9 +200,9 @@ int fann_get_info(const fann_index *ix, fann_info *out);
  * of those events and returns, in milliseconds, the duration of the most recent
  * lookup-table kernel and plan kernel and the summed durations of the dedup
  * launches and of the scan launches (gather + ADC + top-k) of the most recent call;
- * a value is -1 if that kernel has not run since timing was enabled.  When the call
- * ran in several chunks, dedup and scan launches overlap in time, so the two sums
- * can exceed the call's wall time.  Any pointer may be NULL.
+ * a value is -1 if that kernel has not run since timing was enabled.  dedup_ms covers
+ * the partition and the dedup kernels (with FANN_CHUNKS > 1 the partition kernels run on
+ * a second stream under the scans and are not in it).  Any pointer may be NULL.
  */
 int fann_set_timing(fann_index *ix, int enable);
 int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup_ms, float *scan_ms);

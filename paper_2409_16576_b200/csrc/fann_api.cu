@@ -19,7 +19,7 @@ struct fann_index {
     size_t bounce_bytes = 0;
     int num_sms = 0;
     int smem_optin = 0;                    // max dynamic shared memory per block
-    uint32_t chunks = 1;                   // batch chunks: dedup of chunk i+1 runs beside the scan of chunk i
+    uint32_t chunks = 1;                   // batch chunks (FANN_CHUNKS): partition of chunk i+1 runs beside the scan of chunk i
     uint32_t force_mode = 2;               // dedup placement: 0 ordered, 1 hashed, 2 decided per query (FANN_DEDUP_MODE)
     uint32_t scan_ring = 3;                // scan kernel: stages of the per-warp code-row ring, 0 = rows through registers (FANN_SCAN_RING)
     bool partition = true;                 // split lists into their dedup classes first (FANN_PARTITION=0: filter per pass)
@@ -358,9 +358,7 @@ static int scan_ctas_per_sm(const fann_index *ix, size_t smem)
     return (e == cudaSuccess && n >= 1) ? n : 1;
 }
 
-// plan + dedup (+ scan unless dump).  With chunks > 1 the dedup launches go to the index's side
-// stream and the scan of chunk i waits only for the dedup of chunk i, so the HBM-bound scan and
-// the shared-memory-bound dedup of the next chunk share the SMs.
+// plan + mode + partition + dedup (+ scan unless dump), chunk of queries by chunk (one chunk by default).
 static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     const int64_t *cand_offsets, const uint32_t *cand_ids, uint64_t total_cands,
                     uint32_t k, uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
@@ -398,7 +396,6 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     uint32_t chunks = dump ? 1u : ix->chunks;
     if (chunks > B) chunks = B;
     const bool overlap = chunks > 1;
-    cudaStream_t dstream = overlap ? ix->side : stream;
     if (overlap) {
         CUDA_TRY(cudaEventRecord(ix->ev_fork, stream));
         CUDA_TRY(cudaStreamWaitEvent(ix->side, ix->ev_fork, 0));
@@ -410,57 +407,62 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     dp.uniq_ids = uniq_ids; dp.uniq_counts = uniq_counts;
     dp.part_ids = ix->partition ? (const uint32_t *)(ws + w.part_ids) : nullptr;
     dp.part_ok = (const uint32_t *)(ws + w.part_ok); dp.bucket_cnt = (const uint32_t *)(ws + w.bucket_cnt);
-    if (timing) cudaEventRecord(ix->ev_dedup[0][0], dstream);
-    if (ix->partition) {
-        PartParams pp;
-        pp.cand_offsets = (const long long *)cand_offsets; pp.cand_ids = cand_ids; pp.N = ix->N;
-        pp.S = S; pp.mode = mode; pp.item_start = item_start;
-        pp.part_ids = (uint32_t *)(ws + w.part_ids); pp.part_ok = (uint32_t *)(ws + w.part_ok);
-        pp.bucket_cnt = (uint32_t *)(ws + w.bucket_cnt);
-        partition_kernel<<<B, kPartThreads, 0, dstream>>>(pp);
-        ix->launches++;
-        CUDA_TRY(cudaGetLastError());
-    }
+    PartParams pp;
+    pp.cand_offsets = (const long long *)cand_offsets; pp.cand_ids = cand_ids; pp.N = ix->N;
+    pp.S = S; pp.mode = mode; pp.item_start = item_start;
+    pp.part_ids = (uint32_t *)(ws + w.part_ids); pp.part_ok = (uint32_t *)(ws + w.part_ok);
+    pp.bucket_cnt = (uint32_t *)(ws + w.bucket_cnt);
     ScanParams sp;
     sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
     sp.out_ids = out_ids; sp.out_dists = out_dists; sp.out_counts = out_counts; sp.out_uniq = out_uniq;
     const int per_sm = dump ? 1 : scan_ctas_per_sm(ix, g.scan_smem);
 
+    // With chunks > 1 the partition launches of all chunks go to the side stream at once: the partition kernel is
+    // HBM-bound, light on registers and shared memory, and fits on an SM beside a scan CTA, so the split of chunk
+    // c + 1 runs under the scan of chunk c.  Dedup and scan stay on `stream`, chunk by chunk.
+    if (overlap && ix->partition) {
+        for (uint32_t c = 0; c < chunks; ++c) {
+            const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
+            pp.q_begin = qb;
+            partition_kernel<<<qe - qb, kPartThreads, 0, ix->side>>>(pp);
+            ix->launches++;
+            CUDA_TRY(cudaGetLastError());
+            CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], ix->side));
+        }
+    }
     for (uint32_t c = 0; c < chunks; ++c) {
         const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
+        if (overlap && ix->partition) CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_dedup_done[c], 0));
+        if (timing) cudaEventRecord(ix->ev_dedup[c][0], stream);
+        if (!overlap && ix->partition) {
+            pp.q_begin = 0;
+            partition_kernel<<<B, kPartThreads, 0, stream>>>(pp);
+            ix->launches++;
+            CUDA_TRY(cudaGetLastError());
+        }
         dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
-        if (timing && c > 0) cudaEventRecord(ix->ev_dedup[c][0], dstream);
-        if (g.dedup_threads == 512) dedup_kernel<512><<<2 * ix->num_sms, 512, g.dedup_smem, dstream>>>(dp);
-        else dedup_kernel<1024><<<ix->num_sms, 1024, g.dedup_smem, dstream>>>(dp);
-        if (timing) cudaEventRecord(ix->ev_dedup[c][1], dstream);
+        if (g.dedup_threads == 512) dedup_kernel<512><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
+        else dedup_kernel<1024><<<ix->num_sms, 1024, g.dedup_smem, stream>>>(dp);
+        if (timing) cudaEventRecord(ix->ev_dedup[c][1], stream);
         ix->launches++;
         CUDA_TRY(cudaGetLastError());
-        if (overlap) CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], dstream));
+        if (dump) continue;
+        sp.q_begin = qb; sp.q_end = qe; sp.counter = &hdr->scan_counter[c];
+        int grid = ix->num_sms * per_sm;
+        if ((uint32_t)grid > qe - qb) grid = (int)(qe - qb);
+        if (timing) cudaEventRecord(ix->ev_scan[c][0], stream);
+        cudaError_t e = launch_scan(ix, grid, g.scan_smem, stream, sp);
+        if (timing) cudaEventRecord(ix->ev_scan[c][1], stream);
+        ix->launches++;
+        if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
+        ix->last_scan_ctas = (uint32_t)grid;
     }
     ix->last_dedup_threads = g.dedup_threads; ix->last_dedup_smem = g.dedup_smem;
     ix->last_dedup_ctas = (uint32_t)ix->num_sms * (1024u / g.dedup_threads); ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
-    ix->timed_chunks = timing ? chunks : 0; ix->timed_scan = false;
-    if (!dump) {
-        for (uint32_t c = 0; c < chunks; ++c) {
-            const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
-            sp.q_begin = qb; sp.q_end = qe; sp.counter = &hdr->scan_counter[c];
-            int grid = ix->num_sms * per_sm;
-            if ((uint32_t)grid > qe - qb) grid = (int)(qe - qb);
-            if (overlap) CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_dedup_done[c], 0));
-            if (timing) cudaEventRecord(ix->ev_scan[c][0], stream);
-            cudaError_t e = launch_scan(ix, grid, g.scan_smem, stream, sp);
-            if (timing) cudaEventRecord(ix->ev_scan[c][1], stream);
-            ix->launches++;
-            if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
-            ix->last_scan_ctas = (uint32_t)grid;
-        }
-        ix->last_scan_smem = g.scan_smem; ix->last_cap = g.cap;
-        ix->timed_scan = timing;
-    } else if (overlap) {
-        CUDA_TRY(cudaEventRecord(ix->ev_join, dstream));
-        CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_join, 0));
-    }
+    ix->timed_chunks = timing ? chunks : 0;
+    ix->last_scan_smem = g.scan_smem; ix->last_cap = g.cap;
+    ix->timed_scan = timing && !dump;
     ix->have_scan = timing;
     return FANN_OK;
 }

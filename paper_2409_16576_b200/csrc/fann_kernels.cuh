@@ -335,6 +335,7 @@ struct PartParams {
     uint32_t *part_ids;                              // query b's buckets at 2 * cand_offsets[b], bucket p at p * cap_b
     uint32_t *part_ok;                               // [B]
     uint32_t *bucket_cnt;                            // [n_items]
+    uint32_t q_begin;                                // first query of this launch (one CTA per query)
 };
 
 // Splits the candidate list of every query that needs S >= 2 dedup partitions into its S classes, so that
@@ -344,7 +345,7 @@ struct PartParams {
 __global__ void __launch_bounds__(kPartThreads) partition_kernel(const PartParams p)
 {
     __shared__ uint32_t scnt[kMaxPartBuckets];
-    const uint32_t b = blockIdx.x, tid = threadIdx.x, lane = tid & 31;
+    const uint32_t b = p.q_begin + blockIdx.x, tid = threadIdx.x, lane = tid & 31;
     const uint32_t S = p.S[b];
     if (S < 2 || S > kMaxPartBuckets) { if (tid == 0) p.part_ok[b] = 0; return; }
     const bool hashed = p.mode[b] == kModeHashed;
