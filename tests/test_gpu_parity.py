@@ -269,6 +269,17 @@ def test_fp32_config_band(fann, w_f32):
     band_all(w_f32, res)
 
 
+@pytest.mark.parametrize("d,M", [(15, 5), (7, 7), (40, 40), (34, 17), (130, 26)])
+def test_odd_geometries_band(fann, d, M):
+    """PQ shapes outside BASELINE's five: M that does not fill a stored row (padding bytes must not
+    contribute), dsub without the float4 table path, rows of 16, 32 and 64 bytes."""
+    cfg = CONFIGS["tiny_local"].scaled(name=f"odd_d{d}_M{M}", N=60_000, n_lists=600, B=10, d=d, M=M, k=50)
+    w = make_workload(cfg)
+    _, lut, res = gpu_search(fann, w)
+    check_lut(lut.cpu().numpy(), oracle.build_lut(w.queries.numpy(), w.codebooks.numpy()))
+    band_all(w, res)
+
+
 def test_edge_cases(fann, w_int):
     w = w_int
     N = w.cfg.N
