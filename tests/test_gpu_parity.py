@@ -280,6 +280,37 @@ def test_odd_geometries_band(fann, d, M):
     band_all(w, res)
 
 
+def test_table_overflow_is_reported_not_silent(fann, monkeypatch):
+    """Ordered placement FORCED on a list the library itself would hash (60,000 distinct IDs bunched into
+    6 % of [0, N)): one ID-range class receives more distinct IDs than a table has slots.  The call must
+    report FANN_EOVERFLOW through fann_workspace_status instead of returning a wrong answer quietly; the
+    library's own choice (hashed placement) handles the same list exactly."""
+    import paper_2409_16576_b200 as f
+    N, M = 1_000_000, 16
+    ids = np.random.default_rng(3).permutation(60_000).astype(np.uint32)
+    off = np.array([0, ids.size], dtype=np.int64)
+    codes = torch.zeros((N, M), dtype=torch.uint8, device=DEV)
+    o = torch.from_numpy(off).to(DEV)
+    i = torch.from_numpy(ids.view(np.int32)).to(DEV)
+    lut = torch.zeros((1, M, 256), dtype=torch.float32, device=DEV)
+    for force, expect_overflow in (("0", True), (None, False)):
+        if force is None:
+            monkeypatch.delenv("FANN_DEDUP_MODE", raising=False)
+        else:
+            monkeypatch.setenv("FANN_DEDUP_MODE", force)
+        ix = f.FannIndex(0)
+        ix.load_codes(codes)
+        if expect_overflow:
+            with pytest.raises(f.FannError) as err:
+                ix.dedup_scan_topk(lut, o, i, 10, check=True)
+            assert err.value.code == -6                       # FANN_EOVERFLOW
+        else:
+            out = ix.dedup_scan_topk(lut, o, i, 10, check=True)
+            torch.cuda.synchronize()
+            assert int(out[3][0]) == 60_000 and np.array_equal(np_u32(out[0])[0], np.arange(10, dtype=np.uint32))
+        ix.close()
+
+
 def test_edge_cases(fann, w_int):
     w = w_int
     N = w.cfg.N
