@@ -29,6 +29,13 @@
  *     FANN_ID_NONE in a candidate list is skipped; an ID >= N is dropped.
  *   - There is no CPU fallback.  If no usable CUDA device exists the calls
  *     fail with FANN_ECUDA.
+ *   - Alignment: lut 16 bytes; cand_offsets and list offsets 8 bytes; every other array 4
+ *     bytes; workspaces 256 bytes.  A misaligned pointer is FANN_EINVAL / FANN_EWORKSPACE.
+ *   - Threads ("each CPU thread handles an individual query"): once the codes
+ *     (and posting lists / raw vectors) are loaded, any number of host threads may call the
+ *     search entry points on ONE handle at the same time, each with its own stream,
+ *     workspace and output arrays.  The loaders, fann_set_timing and fann_destroy must not
+ *     run beside any other call on the handle; with timing enabled, calls are serialised.
  */
 #ifndef FANN_H
 #define FANN_H
@@ -146,9 +153,16 @@ int fann_dedup_only(fann_index *ix, uint32_t B, const int64_t *cand_offsets,
 
 /*
  * Synchronises `stream` and returns the status the last fann_dedup_scan_topk /
- * fann_dedup_only left in `workspace`: FANN_OK, or FANN_EOVERFLOW if some
- * query's dedup table filled up (only possible for candidate IDs chosen to
- * collide under the library's hash; that query's outputs are then invalid).
+ * fann_dedup_only left in `workspace`:
+ *   FANN_OK
+ *   FANN_EINVAL     total_cands did not match cand_offsets (cand_offsets[0] != 0 or
+ *                   cand_offsets[B] != total_cands): nothing was read or scored, every
+ *                   query reports zero candidates
+ *   FANN_EOVERFLOW  some query's dedup table filled up; that query's outputs are invalid.
+ *                   Candidate lists whose IDs are bunched in part of [0, N) are handled
+ *                   exactly (the library counts the ID-range classes and falls back to hash
+ *                   classes); an overflow is left only for IDs chosen to collide under the
+ *                   library's hash function.
  */
 int fann_workspace_status(fann_index *ix, const void *workspace, void *stream);
 
@@ -190,6 +204,7 @@ typedef struct fann_info {
     uint32_t chunks;           /* batch chunks of the last call (1 unless FANN_CHUNKS is set) */
     uint32_t reserved;
     uint64_t kernel_launches;  /* kernels this index has launched so far                      */
+    uint64_t codes_device_ptr; /* device address of the stored code array [N][row_bytes]      */
 } fann_info;
 int fann_get_info(const fann_index *ix, fann_info *out);
 
@@ -206,19 +221,6 @@ int fann_get_info(const fann_index *ix, fann_info *out);
  */
 int fann_set_timing(fann_index *ix, int enable);
 int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup_ms, float *scan_ms);
-
-/*
- * Measurement only: read the stored code rows of
- * ids[0 .. n) with the scan kernel's access pattern (the same lanes per row, loads
- * in flight and threads per CTA) and do nothing else.  Timed by the caller, it
- * gives the rate at which this GPU can gather those rows at all -- the practical
- * ceiling of step (6).  IDs >= N read row 0.
- * flavor bits 0-7: load instruction (0 plain 16-byte non-coherent loads, 1 the scan kernel's: the same with a 64-byte
- * L2 fetch, 2-5 other cache hints, 6-7 32-byte loads); bits 8 and up: CTAs per SM (0 = 2).
- * ids  device, [n] uint32      sink  device, 4 bytes (never written in practice)
- */
-int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink,
-                      uint32_t flavor, void *stream);
 
 #ifdef __cplusplus
 }

@@ -1,4 +1,7 @@
-"""Parity rules between the CUDA path and the oracle."""
+"""Parity rules between the CUDA path and the oracle.
+
+TEST INFRASTRUCTURE like the rest of oracle/: used by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline leg to compare what the CUDA path returned with what the oracle computed."""
 import numpy as np
 
 NONE = 0xFFFFFFFF

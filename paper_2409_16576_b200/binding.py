@@ -35,7 +35,7 @@ class _Info(C.Structure):
                 ("dedup_threads", C.c_uint32), ("dedup_ctas", C.c_uint32), ("dedup_smem_bytes", C.c_uint32),
                 ("table_slots", C.c_uint32), ("scan_threads", C.c_uint32), ("scan_ctas", C.c_uint32),
                 ("scan_smem_bytes", C.c_uint32), ("scan_buffer_keys", C.c_uint32), ("chunks", C.c_uint32),
-                ("reserved", C.c_uint32), ("kernel_launches", C.c_uint64)]
+                ("reserved", C.c_uint32), ("kernel_launches", C.c_uint64), ("codes_device_ptr", C.c_uint64)]
 
 
 def library_path() -> str:
@@ -69,7 +69,6 @@ def load_library():
         "fann_get_info": (i, [p, C.POINTER(_Info)]),
         "fann_set_timing": (i, [p, i]),
         "fann_last_timing": (i, [p] + [C.POINTER(C.c_float)] * 4),
-        "fann_gather_probe": (i, [p, p, u64, p, u32, p]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -179,10 +178,6 @@ def fann_last_timing(ix) -> dict:
     v = [C.c_float(-1.0) for _ in range(4)]
     _check(load_library().fann_last_timing(ix, *[C.byref(x) for x in v]))
     return dict(zip(("lut_ms", "plan_ms", "dedup_ms", "scan_ms"), (float(x.value) for x in v)))
-
-
-def fann_gather_probe(ix, ids, n, sink, flavor=0, stream=None) -> None:
-    _check(load_library().fann_gather_probe(ix, _addr(ids), n, _addr(sink), flavor, stream))
 
 
 # ---- convenience wrapper (torch for device memory and streams only) ----------

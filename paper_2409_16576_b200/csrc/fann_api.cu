@@ -3,12 +3,24 @@
 #include "../../include/fann.h"
 #include "fann_kernels.cuh"
 
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
+#include <vector>
 
 using namespace fann;
+
+// What one call needs besides the caller's stream: a second stream and events for the transfer / partition overlap.
+// Calls take one from the index's pool and give it back on return, so concurrent calls on one handle (different
+// host threads, streams and workspaces; "each CPU thread handles an individual query") never share
+// an event between a record and its wait.
+struct CallCtx {
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_done[kMaxChunks] = {};
+};
 
 struct fann_index {
     int device = 0;
@@ -26,14 +38,15 @@ struct fann_index {
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint32_t dedup_smem_half = 0;          // same for two CTAs per SM
     uint32_t dedup_threads = 0;            // 0: chosen per call (geometry()); 1024 or 512: forced (FANN_DEDUP_THREADS)
-    uint64_t launches = 0;
-    // second stream + events for the dedup/scan overlap
-    cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_dedup_done[kMaxChunks] = {}, ev_join = nullptr;
+    std::atomic<uint64_t> launches{0};
+    // everything below is shared by concurrent callers and guarded by `mu`
+    std::mutex mu;
+    std::vector<CallCtx *> ctx_pool;       // idle call contexts
     // geometry of the last launches (fann_get_info)
     uint32_t last_dedup_threads = 1024, last_dedup_smem = 0, last_dedup_ctas = 0, last_scan_ctas = 0, last_scan_smem = 0, last_cap = 0, last_slots = 0, last_chunks = 0;
-    // optional per-kernel timing
-    bool timing = false;
+    // optional per-kernel timing (benchmarks; timed calls are serialised by `timing_mu`)
+    std::mutex timing_mu;
+    std::atomic<bool> timing{false};
     cudaEvent_t ev_lut[2] = {}, ev_plan[2] = {}, ev_dedup[kMaxChunks][2] = {}, ev_scan[kMaxChunks][2] = {};
     bool have_lut = false, have_scan = false;
     uint32_t timed_chunks = 0;
@@ -66,6 +79,41 @@ struct DeviceGuard {
 };
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static void destroy_ctx(CallCtx *c)
+{
+    if (!c) return;
+    if (c->side) cudaStreamDestroy(c->side);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    for (auto &e : c->ev_done) if (e) cudaEventDestroy(e);
+    delete c;
+}
+
+// RAII: a call context from the index's pool (created on first use), returned on scope exit.
+struct CtxLease {
+    fann_index *ix;
+    CallCtx *c = nullptr;
+    explicit CtxLease(fann_index *ix_) : ix(ix_)       // ix_ == NULL: the call needs no second stream
+    {
+        if (!ix) return;
+        {
+            std::lock_guard<std::mutex> g(ix->mu);
+            if (!ix->ctx_pool.empty()) { c = ix->ctx_pool.back(); ix->ctx_pool.pop_back(); }
+        }
+        if (c) return;
+        c = new CallCtx();
+        bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+        for (auto &e : c->ev_done) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) { destroy_ctx(c); c = nullptr; }
+    }
+    ~CtxLease()
+    {
+        if (!c) return;
+        std::lock_guard<std::mutex> g(ix->mu);
+        ix->ctx_pool.push_back(c);
+    }
+};
 
 // ---------------------------------------------------------------- geometry + workspace layout
 
@@ -159,31 +207,19 @@ extern "C" int fann_create(fann_index **out, int device)
     CUDA_TRY((set_scan_attr<1, 4, 3>(ring_max)));
     CUDA_TRY((set_scan_attr<2, 4, 3>(ring_max)));
     CUDA_TRY((set_scan_attr<4, 2, 3>(ring_max)));
+    int per_sm = 0;
+    CUDA_TRY(cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device));
     fann_index *ix = new fann_index();
     ix->device = device; ix->num_sms = num_sms; ix->smem_optin = smem_optin;
     ix->dedup_smem = (uint32_t)smem_optin;
+    // two dedup CTAs per SM: each gets half of the SM's shared memory less the 1 KB the driver reserves per CTA
+    ix->dedup_smem_half = (uint32_t)((per_sm / 2 - 1024) & ~255);
+    // A/B knobs (DESIGN.md 6.4 "Knobs"); the defaults are the product, tests run every alternative
     if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
     if (const char *s = getenv("FANN_PARTITION")) ix->partition = atoi(s) != 0;
     if (const char *s = getenv("FANN_SCAN_RING")) { int v = atoi(s); if (v == 0 || v == 3) ix->scan_ring = (uint32_t)v; }
-    if (const char *s = getenv("FANN_L2_FETCH")) {
-        int v = atoi(s);
-        if (v == 32 || v == 64 || v == 128) CUDA_TRY(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)v));
-    }
-    {   // two dedup CTAs per SM: each gets half of the SM's shared memory less the 1 KB the driver reserves per CTA
-        int per_sm = 0;
-        CUDA_TRY(cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device));
-        ix->dedup_smem_half = (uint32_t)((per_sm / 2 - 1024) & ~255);
-    }
     if (const char *s = getenv("FANN_DEDUP_THREADS")) { int v = atoi(s); if (v == 512 || v == 1024) ix->dedup_threads = (uint32_t)v; }
-    if (const char *s = getenv("FANN_DEDUP_SMEM_KB")) {
-        int v = atoi(s) * 1024;
-        if (v >= 16 * 1024 && v <= smem_optin) ix->dedup_smem = (uint32_t)v;
-    }
-    CUDA_TRY(cudaStreamCreateWithFlags(&ix->side, cudaStreamNonBlocking));
-    CUDA_TRY(cudaEventCreateWithFlags(&ix->ev_fork, cudaEventDisableTiming));
-    CUDA_TRY(cudaEventCreateWithFlags(&ix->ev_join, cudaEventDisableTiming));
-    for (auto &ev : ix->ev_dedup_done) CUDA_TRY(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
     *out = ix;
     return FANN_OK;
 }
@@ -195,10 +231,7 @@ extern "C" void fann_destroy(fann_index *ix)
     cudaDeviceSynchronize();
     if (ix->codes) cudaFree(ix->codes);
     if (ix->bounce) cudaFree(ix->bounce);
-    if (ix->side) cudaStreamDestroy(ix->side);
-    if (ix->ev_fork) cudaEventDestroy(ix->ev_fork);
-    if (ix->ev_join) cudaEventDestroy(ix->ev_join);
-    for (auto &e : ix->ev_dedup_done) if (e) cudaEventDestroy(e);
+    for (CallCtx *c : ix->ctx_pool) destroy_ctx(c);
     for (auto &e : ix->ev_lut) if (e) cudaEventDestroy(e);
     for (auto &e : ix->ev_plan) if (e) cudaEventDestroy(e);
     for (auto &c : ix->ev_dedup) for (auto &e : c) if (e) cudaEventDestroy(e);
@@ -209,6 +242,9 @@ extern "C" void fann_destroy(fann_index *ix)
 extern "C" int fann_get_info(const fann_index *ix, fann_info *out)
 {
     if (!ix || !out) return fail(FANN_EINVAL, "fann_get_info: NULL argument");
+    std::lock_guard<std::mutex> g(const_cast<fann_index *>(ix)->mu);
+    out->codes_device_ptr = (uint64_t)(uintptr_t)ix->codes;
+    out->reserved = 0;
     out->N = ix->N; out->M = ix->M; out->row_bytes = ix->row_bytes;
     out->num_sms = (uint32_t)ix->num_sms;
     out->dedup_threads = ix->last_dedup_threads; out->dedup_ctas = ix->last_dedup_ctas;
@@ -216,7 +252,7 @@ extern "C" int fann_get_info(const fann_index *ix, fann_info *out)
     out->scan_threads = kScanThreads; out->scan_ctas = ix->last_scan_ctas;
     out->scan_smem_bytes = ix->last_scan_smem; out->scan_buffer_keys = ix->last_cap;
     out->chunks = ix->last_chunks;
-    out->kernel_launches = ix->launches;
+    out->kernel_launches = ix->launches.load();
     return FANN_OK;
 }
 
@@ -303,13 +339,19 @@ extern "C" int fann_build_lut(fann_index *ix, const float *queries, uint32_t B,
     cudaStream_t stream = (cudaStream_t)stream_;
     const uint64_t blocks = (uint64_t)B * ((ix->M + 3) / 4);
     if (blocks > 0x7FFFFFFFull) return fail(FANN_EUNSUPPORTED, "fann_build_lut: B=%u too large for one launch", B);
+    if (((uintptr_t)lut & 15) != 0) return fail(FANN_EINVAL, "fann_build_lut: lut must be 16-byte aligned");
+    if ((((uintptr_t)queries | (uintptr_t)codebooks) & 3) != 0)
+        return fail(FANN_EINVAL, "fann_build_lut: queries and codebooks must be 4-byte aligned");
     const bool vec = (((uintptr_t)codebooks | (uintptr_t)queries) & 15) == 0;   // float4 reads of the codebook
-    if (ix->timing) cudaEventRecord(ix->ev_lut[0], stream);
+    const bool timing = ix->timing.load();
+    std::unique_lock<std::mutex> tl(ix->timing_mu, std::defer_lock);
+    if (timing) tl.lock();
+    if (timing) cudaEventRecord(ix->ev_lut[0], stream);
     if (vec && dsub == 2) build_lut_kernel<2><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
     else if (vec && dsub == 4) build_lut_kernel<4><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
     else if (vec && dsub == 8) build_lut_kernel<8><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
     else build_lut_kernel<0><<<(unsigned)blocks, 256, 0, stream>>>(queries, codebooks, lut, ix->M, dsub);
-    if (ix->timing) { cudaEventRecord(ix->ev_lut[1], stream); ix->have_lut = true; }
+    if (timing) { cudaEventRecord(ix->ev_lut[1], stream); ix->have_lut = true; }
     ix->launches++;
     CUDA_TRY(cudaGetLastError());
     return FANN_OK;
@@ -359,12 +401,14 @@ static int scan_ctas_per_sm(const fann_index *ix, size_t smem)
 }
 
 // plan + mode + partition + dedup (+ scan unless dump), chunk of queries by chunk (one chunk by default).
+// exact_total: the call covers the whole CSR (cand_offsets[0] == 0, cand_offsets[B] == total_cands); a chunk of a
+// larger batch (fann_search_host) passes absolute offsets into the whole ID array instead.
 static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     const int64_t *cand_offsets, const uint32_t *cand_ids, uint64_t total_cands,
                     uint32_t k, uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
                     uint32_t *out_uniq, uint32_t *uniq_ids, uint32_t *uniq_counts,
                     void *workspace, size_t workspace_bytes, cudaStream_t stream,
-                    uint32_t shape = 0, bool keep_status = false)
+                    uint32_t shape = 0, bool keep_status = false, bool exact_total = true)
 {
     Geom g;
     geometry(ix, k, B, total_cands, &g, shape);
@@ -374,6 +418,11 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         return fail(FANN_EWORKSPACE, "workspace is NULL or not 256-byte aligned");
     if (workspace_bytes < w.total)
         return fail(FANN_EWORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, w.total);
+    if (((uintptr_t)cand_offsets & 7) != 0) return fail(FANN_EINVAL, "cand_offsets must be 8-byte aligned");
+    if ((((uintptr_t)cand_ids | (uintptr_t)out_ids | (uintptr_t)out_dists | (uintptr_t)out_counts |
+          (uintptr_t)out_uniq | (uintptr_t)uniq_ids | (uintptr_t)uniq_counts) & 3) != 0)
+        return fail(FANN_EINVAL, "ID and output arrays must be 4-byte aligned");
+    if (lut && ((uintptr_t)lut & 15) != 0) return fail(FANN_EINVAL, "lut must be 16-byte aligned");
     DeviceGuard guard(ix->device);
     char *ws = (char *)workspace;
     WsHeader *hdr = (WsHeader *)(ws + w.hdr);
@@ -383,22 +432,28 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     uint2 *items = (uint2 *)(ws + w.items);
     if (!dump) { uniq_counts = (uint32_t *)(ws + w.uniq_counts); uniq_ids = (uint32_t *)(ws + w.uniq_ids); }
 
-    const bool timing = ix->timing;
+    const bool timing = ix->timing.load();
+    std::unique_lock<std::mutex> tl(ix->timing_mu, std::defer_lock);
+    if (timing) tl.lock();
     if (timing) cudaEventRecord(ix->ev_plan[0], stream);
     plan_kernel<<<1, 1024, 0, stream>>>((const long long *)cand_offsets, B, g.cap_c, w.max_items, hdr, S,
-                                        item_start, items, uniq_counts, keep_status ? 1u : 0u);
+                                        item_start, items, uniq_counts, keep_status ? 1u : 0u,
+                                        (unsigned long long)total_cands, exact_total ? 1u : 0u);
     mode_kernel<<<(B + 7) / 8, 256, 0, stream>>>((const long long *)cand_offsets, cand_ids, B, ix->N,
-                                                  ix->force_mode, mode);
+                                                  ix->force_mode, ix->partition ? 0u : g.cap_c, mode);
     if (timing) cudaEventRecord(ix->ev_plan[1], stream);
     ix->launches += 2;
     CUDA_TRY(cudaGetLastError());
 
     uint32_t chunks = dump ? 1u : ix->chunks;
     if (chunks > B) chunks = B;
-    const bool overlap = chunks > 1;
+    const bool overlap = chunks > 1 && ix->partition;
+    CtxLease lease(overlap ? ix : nullptr);                    // returned to the pool when the call returns
+    CallCtx *cx = lease.c;
     if (overlap) {
-        CUDA_TRY(cudaEventRecord(ix->ev_fork, stream));
-        CUDA_TRY(cudaStreamWaitEvent(ix->side, ix->ev_fork, 0));
+        if (!cx) return fail(FANN_ECUDA, "could not create the second stream of the call");
+        CUDA_TRY(cudaEventRecord(cx->ev_fork, stream));
+        CUDA_TRY(cudaStreamWaitEvent(cx->side, cx->ev_fork, 0));
     }
 
     DedupParams dp;
@@ -412,6 +467,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     pp.S = S; pp.mode = mode; pp.item_start = item_start;
     pp.part_ids = (uint32_t *)(ws + w.part_ids); pp.part_ok = (uint32_t *)(ws + w.part_ok);
     pp.bucket_cnt = (uint32_t *)(ws + w.bucket_cnt);
+    pp.class_max = (uint32_t)((uint64_t)g.nslots_max * 9 / 10);
     ScanParams sp;
     sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
@@ -421,21 +477,22 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     // With chunks > 1 the partition launches of all chunks go to the side stream at once: the partition kernel is
     // HBM-bound, light on registers and shared memory, and fits on an SM beside a scan CTA, so the split of chunk
     // c + 1 runs under the scan of chunk c.  Dedup and scan stay on `stream`, chunk by chunk.
-    if (overlap && ix->partition) {
+    if (overlap) {
         for (uint32_t c = 0; c < chunks; ++c) {
             const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
             pp.q_begin = qb;
-            partition_kernel<<<qe - qb, kPartThreads, 0, ix->side>>>(pp);
+            partition_kernel<<<qe - qb, kPartThreads, 0, cx->side>>>(pp);
             ix->launches++;
             CUDA_TRY(cudaGetLastError());
-            CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], ix->side));
+            CUDA_TRY(cudaEventRecord(cx->ev_done[c], cx->side));
         }
     }
+    uint32_t scan_ctas = 0;
     for (uint32_t c = 0; c < chunks; ++c) {
         const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
-        if (overlap && ix->partition) CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_dedup_done[c], 0));
+        if (overlap) CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_done[c], 0));
         if (timing) cudaEventRecord(ix->ev_dedup[c][0], stream);
-        if (!overlap && ix->partition) {
+        if (!overlap && ix->partition && c == 0) {
             pp.q_begin = 0;
             partition_kernel<<<B, kPartThreads, 0, stream>>>(pp);
             ix->launches++;
@@ -456,14 +513,20 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         if (timing) cudaEventRecord(ix->ev_scan[c][1], stream);
         ix->launches++;
         if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
-        ix->last_scan_ctas = (uint32_t)grid;
+        scan_ctas = (uint32_t)grid;
     }
-    ix->last_dedup_threads = g.dedup_threads; ix->last_dedup_smem = g.dedup_smem;
-    ix->last_dedup_ctas = (uint32_t)ix->num_sms * (1024u / g.dedup_threads); ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
-    ix->timed_chunks = timing ? chunks : 0;
-    ix->last_scan_smem = g.scan_smem; ix->last_cap = g.cap;
-    ix->timed_scan = timing && !dump;
-    ix->have_scan = timing;
+    {
+        std::lock_guard<std::mutex> lg(ix->mu);
+        if (scan_ctas) ix->last_scan_ctas = scan_ctas;
+        ix->last_dedup_threads = g.dedup_threads; ix->last_dedup_smem = g.dedup_smem;
+        ix->last_dedup_ctas = (uint32_t)ix->num_sms * (1024u / g.dedup_threads); ix->last_slots = g.nslots_max; ix->last_chunks = chunks;
+        ix->last_scan_smem = g.scan_smem; ix->last_cap = g.cap;
+    }
+    if (timing) {
+        ix->timed_chunks = chunks;
+        ix->timed_scan = !dump;
+        ix->have_scan = true;
+    }
     return FANN_OK;
 }
 
@@ -579,20 +642,23 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
     Geom g;
     geometry(ix, k, B, total, &g);                             // one dedup CTA shape for all chunks: the layout depends on it
     const uint32_t nchunk = (B >= 64 && total >= (4u << 20) && ix->chunks == 1) ? 8u : 1u;   // 16 MB of IDs and up
-    CUDA_TRY(cudaEventRecord(ix->ev_fork, stream));
-    CUDA_TRY(cudaStreamWaitEvent(ix->side, ix->ev_fork, 0));   // the scratch may still be in use by earlier work on `stream`
+    CtxLease lease(ix);
+    CallCtx *cx = lease.c;
+    if (!cx) return fail(FANN_ECUDA, "fann_search_host: could not create the transfer stream");
+    CUDA_TRY(cudaEventRecord(cx->ev_fork, stream));
+    CUDA_TRY(cudaStreamWaitEvent(cx->side, cx->ev_fork, 0));   // the scratch may still be in use by earlier work on `stream`
     for (uint32_t c = 0; c < nchunk; ++c) {
         const uint32_t b0 = (uint32_t)((uint64_t)B * c / nchunk), b1 = (uint32_t)((uint64_t)B * (c + 1) / nchunk);
         const uint64_t e0 = (uint64_t)cand_offsets_h[b0], e1 = (uint64_t)cand_offsets_h[b1];
         if (e1 > e0)
-            CUDA_TRY(cudaMemcpyAsync(s + h.ids + e0 * 4, cand_ids_h + e0, (size_t)(e1 - e0) * 4, cudaMemcpyHostToDevice, ix->side));
-        CUDA_TRY(cudaEventRecord(ix->ev_dedup_done[c], ix->side));
-        CUDA_TRY(cudaStreamWaitEvent(stream, ix->ev_dedup_done[c], 0));
+            CUDA_TRY(cudaMemcpyAsync(s + h.ids + e0 * 4, cand_ids_h + e0, (size_t)(e1 - e0) * 4, cudaMemcpyHostToDevice, cx->side));
+        CUDA_TRY(cudaEventRecord(cx->ev_done[c], cx->side));
+        CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_done[c], 0));
         rc = run_path(ix, false, (const float *)(s + h.lut) + (size_t)b0 * ix->M * 256, b1 - b0,
                       (const int64_t *)(s + h.offsets) + b0, (const uint32_t *)(s + h.ids), total, k,
                       (uint32_t *)(s + h.out_ids) + (size_t)b0 * k, (float *)(s + h.out_dists) + (size_t)b0 * k,
                       (uint32_t *)(s + h.out_counts) + b0, nullptr, nullptr, nullptr,
-                      s + h.ws, h.ws_bytes, stream, g.dedup_threads, c > 0);
+                      s + h.ws, h.ws_bytes, stream, g.dedup_threads, c > 0, nchunk == 1);
         if (rc != FANN_OK) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
@@ -605,42 +671,18 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
 
 // ---------------------------------------------------------------- measurement
 
-extern "C" int fann_gather_probe(fann_index *ix, const uint32_t *ids, uint64_t n, uint32_t *sink,
-                                 uint32_t flavor, void *stream_)
-{
-    if (!ix || !ids || !sink) return fail(FANN_EINVAL, "fann_gather_probe: NULL argument");
-    if (!ix->codes) return fail(FANN_EINVAL, "fann_gather_probe: load codes first");
-    const uint32_t mult = flavor >> 8;                  // bits 8..: CTAs per SM (0 = 2), for occupancy sweeps
-    flavor &= 0xffu;
-    if (flavor > 7) return fail(FANN_EINVAL, "fann_gather_probe: flavor %u not in 0..7", flavor);
-    if (flavor >= 6 && ix->row_bytes < 32) return fail(FANN_EUNSUPPORTED, "fann_gather_probe: 32-byte loads need rows >= 32 bytes");
-    DeviceGuard guard(ix->device);
-    cudaStream_t stream = (cudaStream_t)stream_;
-    const int grid = ix->num_sms * (mult ? (int)mult : 2);
-    if (flavor >= 6) {
-        if (ix->row_bytes == 32) gather_probe256_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor);
-        else gather_probe256_kernel<2, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor);
-    } else switch (ix->row_bytes) {
-    case 16: gather_probe_kernel<1, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor); break;
-    case 32: gather_probe_kernel<2, 4><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor); break;
-    default: gather_probe_kernel<4, 2><<<grid, kScanThreads, 0, stream>>>(ix->codes, ids, n, ix->N, sink, flavor); break;
-    }
-    ix->launches++;
-    CUDA_TRY(cudaGetLastError());
-    return FANN_OK;
-}
-
 extern "C" int fann_set_timing(fann_index *ix, int enable)
 {
     if (!ix) return fail(FANN_EINVAL, "fann_set_timing: NULL index");
     DeviceGuard guard(ix->device);
+    std::lock_guard<std::mutex> tl(ix->timing_mu);
     if (enable) {
         for (auto &e : ix->ev_lut) if (!e) CUDA_TRY(cudaEventCreate(&e));
         for (auto &e : ix->ev_plan) if (!e) CUDA_TRY(cudaEventCreate(&e));
         for (auto &c : ix->ev_dedup) for (auto &e : c) if (!e) CUDA_TRY(cudaEventCreate(&e));
         for (auto &c : ix->ev_scan) for (auto &e : c) if (!e) CUDA_TRY(cudaEventCreate(&e));
     }
-    ix->timing = enable != 0;
+    ix->timing.store(enable != 0);
     ix->have_lut = ix->have_scan = false;
     ix->timed_chunks = 0; ix->timed_scan = false;
     return FANN_OK;
@@ -650,6 +692,7 @@ extern "C" int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, f
 {
     if (!ix) return fail(FANN_EINVAL, "fann_last_timing: NULL index");
     DeviceGuard guard(ix->device);
+    std::lock_guard<std::mutex> tl(ix->timing_mu);
     float v[4] = {-1.f, -1.f, -1.f, -1.f};
     if (ix->have_lut) { CUDA_TRY(cudaEventSynchronize(ix->ev_lut[1])); CUDA_TRY(cudaEventElapsedTime(&v[0], ix->ev_lut[0], ix->ev_lut[1])); }
     if (ix->have_scan && ix->timed_chunks) {

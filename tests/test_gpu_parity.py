@@ -7,7 +7,7 @@ import pytest
 import torch
 
 import oracle
-from parity import NONE, check_band, check_exact, check_lut
+from oracle.parity import NONE, check_band, check_exact, check_lut
 from workloads import CONFIGS, make_workload, mini
 
 pytestmark = pytest.mark.gpu
@@ -280,35 +280,111 @@ def test_odd_geometries_band(fann, d, M):
     band_all(w, res)
 
 
-def test_table_overflow_is_reported_not_silent(fann, monkeypatch):
-    """Ordered placement FORCED on a list the library itself would hash (60,000 distinct IDs bunched into
-    6 % of [0, N)): one ID-range class receives more distinct IDs than a table has slots.  The call must
-    report FANN_EOVERFLOW through fann_workspace_status instead of returning a wrong answer quietly; the
-    library's own choice (hashed placement) handles the same list exactly."""
+def _hash_round1(x):
+    """First round of the library's slot hash (fann.h: "IDs chosen to collide under the library's hash")."""
+    x = x.astype(np.uint64)
+    return ((x ^ (x >> np.uint64(16))) * np.uint64(0x7feb352d)) & np.uint64(0xFFFFFFFF)
+
+
+def test_table_overflow_is_reported_not_silent(fann):
+    """IDs CHOSEN to collide: 100,000 distinct IDs whose hash falls into class 0 whatever the number of classes
+    (top four hash bits zero, up to 16 classes).  Neither ID-range classes (the IDs sit in part of [0, N)) nor hash
+    classes can split them, so one table must overflow: the call has to say so through fann_workspace_status,
+    never return a quiet wrong answer."""
     import paper_2409_16576_b200 as f
-    N, M = 1_000_000, 16
-    ids = np.random.default_rng(3).permutation(60_000).astype(np.uint32)
-    off = np.array([0, ids.size], dtype=np.int64)
-    codes = torch.zeros((N, M), dtype=torch.uint8, device=DEV)
+    N, M = 4_000_000, 16
+    allv = np.arange(2_400_000, dtype=np.uint32)
+    ids = allv[(_hash_round1(allv) >> np.uint64(28)) == 0][:100_000]
+    assert ids.size == 100_000
+    ix = f.FannIndex(0)
+    ix.load_codes(torch.zeros((N, M), dtype=torch.uint8, device=DEV))
+    lut = torch.zeros((1, M, 256), dtype=torch.float32, device=DEV)
+    o = torch.from_numpy(np.array([0, ids.size], dtype=np.int64)).to(DEV)
+    i = torch.from_numpy(ids.view(np.int32)).to(DEV)
+    with pytest.raises(f.FannError) as err:
+        ix.dedup_scan_topk(lut, o, i, 10, check=True)
+    assert err.value.code == -6                               # FANN_EOVERFLOW
+    assert ix.info()["table_slots"] < 100_000                 # the premise: one table cannot hold them
+    ix.close()
+
+
+@pytest.mark.parametrize("frac,count", [(0.4, 80_000), (0.5, 160_000), (0.35, 120_000), (0.06, 60_000)])
+def test_dedup_ids_concentrated_in_part_of_the_range(fann, frac, count):
+    """IDs spread evenly over only [0, frac N): no fine-grained bunching for mode_kernel's sample to see, but an
+    ID-range class of the lower part receives far more than its share.  The partition kernel counts the classes
+    exactly and must fall back to hash classes by itself (no FANN_DEDUP_MODE): distinct sets equal the oracle's."""
+    N, M = 2_000_000, 16
+    rng = np.random.default_rng(int(frac * 100) + count)
+    lists = [rng.integers(0, int(frac * N), size=count).astype(np.uint32),
+             rng.permutation(int(frac * N))[:count // 2].astype(np.uint32),
+             rng.integers(0, N, size=count).astype(np.uint32)]                  # an evenly spread list beside them
+    off = np.zeros(len(lists) + 1, dtype=np.int64)
+    off[1:] = np.cumsum([len(x) for x in lists])
+    ids = np.concatenate(lists)
+    ix = fann.FannIndex(0)
+    ix.load_codes(torch.zeros((N, M), dtype=torch.uint8, device=DEV))
     o = torch.from_numpy(off).to(DEV)
     i = torch.from_numpy(ids.view(np.int32)).to(DEV)
-    lut = torch.zeros((1, M, 256), dtype=torch.float32, device=DEV)
-    for force, expect_overflow in (("0", True), (None, False)):
-        if force is None:
-            monkeypatch.delenv("FANN_DEDUP_MODE", raising=False)
-        else:
-            monkeypatch.setenv("FANN_DEDUP_MODE", force)
-        ix = f.FannIndex(0)
-        ix.load_codes(codes)
-        if expect_overflow:
-            with pytest.raises(f.FannError) as err:
-                ix.dedup_scan_topk(lut, o, i, 10, check=True)
-            assert err.value.code == -6                       # FANN_EOVERFLOW
-        else:
-            out = ix.dedup_scan_topk(lut, o, i, 10, check=True)
-            torch.cuda.synchronize()
-            assert int(out[3][0]) == 60_000 and np.array_equal(np_u32(out[0])[0], np.arange(10, dtype=np.uint32))
-        ix.close()
+    uids, ucnt = ix.dedup_only(o, i)                          # raises on FANN_EOVERFLOW
+    torch.cuda.synchronize()
+    uids, ucnt = np_u32(uids), np_u32(ucnt)
+    for b in range(len(lists)):
+        want = oracle.dedup(ids[off[b]:off[b + 1]], N)
+        assert ucnt[b] == want.size
+        assert np.array_equal(np.sort(uids[off[b]:off[b] + ucnt[b]]), want)
+    ix.close()
+
+
+def test_understated_total_cands_is_refused_not_corrupting(fann, w_int):
+    """total_cands is the caller's promise that sized the workspace.  If it does not equal cand_offsets[B] the
+    library must not touch the lists (it would write past its arrays): fann_workspace_status says FANN_EINVAL and
+    every query reports zero candidates."""
+    import paper_2409_16576_b200 as f
+    w = w_int
+    ix = f.FannIndex(0)
+    ix.load_codes(w.codes.to(DEV))
+    lut = ix.build_lut(w.queries.to(DEV), w.codebooks.to(DEV))
+    off, ids = w.cand_offsets.to(DEV), w.cand_ids.to(DEV)
+    B, k = w.cfg.B, 10
+    total = ids.numel()
+    for claimed in (total // 2, total - 1, 1):
+        ws = torch.empty(f.fann_workspace_bytes(ix.handle, B, claimed, k) + 4096, dtype=torch.uint8, device=DEV)
+        ws[-4096:] = 0xAB                                      # canary behind the workspace proper
+        out = (torch.zeros((B, k), dtype=torch.int32, device=DEV), torch.zeros((B, k), device=DEV),
+               torch.full((B,), 77, dtype=torch.int32, device=DEV), torch.full((B,), 77, dtype=torch.int32, device=DEV))
+        f.fann_dedup_scan_topk(ix.handle, lut, B, off, ids, claimed, k, out[0], out[1], out[2], out[3],
+                               ws, ws.numel() - 4096, torch.cuda.current_stream().cuda_stream)
+        with pytest.raises(f.FannError) as err:
+            f.fann_workspace_status(ix.handle, ws, torch.cuda.current_stream().cuda_stream)
+        assert err.value.code == -1                           # FANN_EINVAL
+        assert bool((ws[-4096:] == 0xAB).all())
+        assert bool((out[2] == 0).all()) and bool((out[3] == 0).all()) and bool((out[0] == -1).all())
+    ix.close()
+
+
+def test_misaligned_pointers_are_refused(fann, tiny):
+    import paper_2409_16576_b200 as f
+    w = tiny
+    ix = f.FannIndex(0)
+    ix.load_codes(w.codes.to(DEV))
+    B, M = w.cfg.B, w.cfg.M
+    q, cb = w.queries.to(DEV), w.codebooks.to(DEV)
+    raw = torch.empty(B * M * 256 + 8, dtype=torch.float32, device=DEV)
+    lut_bad = raw[1:1 + B * M * 256]                          # 4-byte aligned only
+    with pytest.raises(f.FannError) as err:
+        f.fann_build_lut(ix.handle, q, B, cb, w.cfg.dsub, lut_bad, None)
+    assert err.value.code == -1
+    lut = ix.build_lut(q, cb)
+    off, ids = w.cand_offsets.to(DEV), w.cand_ids.to(DEV)
+    out = [torch.empty((B, 10), dtype=torch.int32, device=DEV), torch.empty((B, 10), device=DEV)]
+    ws = ix.workspace(B, ids.numel(), 10)
+    torch.cuda.synchronize()
+    lut_copy = raw[1:1 + B * M * 256].copy_(lut.view(-1))
+    with pytest.raises(f.FannError) as err:
+        f.fann_dedup_scan_topk(ix.handle, lut_copy, B, off, ids, ids.numel(), 10, out[0], out[1], None, None,
+                               ws, ws.numel(), None)
+    assert err.value.code == -1
+    ix.close()
 
 
 def test_edge_cases(fann, w_int):
@@ -407,16 +483,17 @@ def test_host_entry_in_chunks_matches_device_entry_and_oracle(fann):
     assert np.array_equal(oi.numpy().view(np.uint32)[:nq], ref["ids"]) and np.array_equal(od.numpy()[:nq], ref["dists"])
 
 
-@pytest.mark.parametrize("name,nq", [("u8_10m_m32", 48), ("u8_1b_m64", 12)])
+@pytest.mark.parametrize("name,nq", [("u8_10m_m32", 48), ("f32_100m_m48", 24), ("i8_1b_m25", 24), ("u8_1b_m64", 12)])
 def test_full_size_configs_sampled_against_oracle(fann, name, nq):
     """BASELINE's configs at full size, in the launch configuration bench.py times (same calls, same
-    workspace sizing): the first nq queries are compared with the oracle byte for byte (integer-exact
-    regime), and every query with properties that hold at any size."""
+    workspace sizing): the first nq queries are compared with the oracle -- lookup tables to 1e-5, results byte
+    for byte in the integer-exact regime and by the tolerance rules for the real-valued config -- and every query
+    with properties that hold at any size."""
     import bench
     cfg = CONFIGS[name]
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
-    if free < 2 * cfg.N * cfg.M + (40 << 30):              # workload's codes + the library's copy + per-batch arrays
+    if free < 2 * cfg.N * max(cfg.M, 32) + (40 << 30):     # workload's codes + the library's copy + per-batch arrays
         pytest.skip("not enough free device memory for this config")
     w = make_workload(cfg, device=DEV)
     B, k = cfg.B, cfg.k
@@ -432,13 +509,83 @@ def test_full_size_configs_sampled_against_oracle(fann, name, nq):
     assert bool((dists[:, 1:] >= dists[:, :-1]).all())
     srt = torch.sort(ids.long() & 0xFFFFFFFF, dim=1).values
     assert bool(((srt[:, 1:] != srt[:, :-1]) | (srt[:, 1:] == 0xFFFFFFFF)).all())
-    # sampled: byte equality with the oracle on the first nq queries
-    _, r, _ = bench.oracle_sample(w, nq, w.codes)
-    assert np.array_equal(np_u32(uniq[:nq]), r["uniq"])
-    assert np.array_equal(np_u32(ids[:nq]), r["ids"]) and np.array_equal(dists[:nq].cpu().numpy(), r["dists"])
+    # sampled: the lookup tables of the first nq queries
+    lut64 = oracle.build_lut(w.queries[:nq].cpu().numpy(), w.codebooks.cpu().numpy())
+    check_lut(lut[:nq].cpu().numpy(), lut64)
+    if cfg.integer_exact:
+        assert np.array_equal(lut[:nq].cpu().numpy().astype(np.float64), lut64)
+        _, r, _ = bench.oracle_sample(w, nq, w.codes)
+        check_exact((np_u32(ids[:nq]), dists[:nq].cpu().numpy(), np_u32(counts[:nq]), np_u32(uniq[:nq])), r)
+    else:
+        bench.band_check_sample(w, nq, w.codes, o)
     ix.close()
     del w, lut, o
     torch.cuda.empty_cache()
+
+
+@pytest.fixture(scope="module")
+def w_m16():
+    """16-byte code rows (M = 16) on integer data: uint8 values, dsub = 8; every ADC sum < 2^24, so bytes compare."""
+    cfg = mini("u8_10m_m32", N=400_000, n_lists=800, B=6, codes_mode="histogram", M=16)
+    assert cfg.M * cfg.dsub * 255 ** 2 < 2 ** 24
+    return make_workload(cfg)
+
+
+@pytest.mark.parametrize("k", [1, 100, 1000, 1024])
+@pytest.mark.parametrize("rows", [16, 32, 64])
+def test_row_bytes_times_k_matrix_bytes(fann, w_m16, w_int, w_k1000, rows, k):
+    """Every stored row size (16 / 32 / 64 bytes: 128 / 64 / 32 rows per ring stage, different buffer margins)
+    against every k regime up to the compiled maximum, U >> k, integer-exact: byte equality with the oracle."""
+    w = {16: w_m16, 32: w_int, 64: w_k1000}[rows]
+    ix, _, res = gpu_search(fann, w, k=k)
+    assert ix.info()["row_bytes"] == rows
+    ref = orc_search(w, k=k)
+    assert ref["uniq"].min() > 4 * k or k >= 1000
+    check_exact(res, ref)
+
+
+def test_two_host_threads_on_one_handle(fann, w_int, w_i8):
+    """PAPER.md:L204 "each CPU thread handles an individual query": two host threads call the path on ONE handle
+    at the same time, each with its own stream, workspace and outputs (fann.h "Threads").  Bytes equal the serial run."""
+    import threading
+    import paper_2409_16576_b200 as f
+    w = w_int
+    ix, _, serial = gpu_search(fann, w)
+    q, cb = w.queries.to(DEV), w.codebooks.to(DEV)
+    off, ids = w.cand_offsets.to(DEV), w.cand_ids.to(DEV)
+    B, k, total = w.cfg.B, w.cfg.k, w.cand_ids.numel()
+    need = f.fann_workspace_bytes(ix.handle, B, total, k)
+    results, errors = {}, []
+
+    def worker(t):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                ws = torch.empty(need, dtype=torch.uint8, device=DEV)
+                lut = torch.empty((B, w.cfg.M, 256), dtype=torch.float32, device=DEV)
+                out = (torch.empty((B, k), dtype=torch.int32, device=DEV), torch.empty((B, k), device=DEV),
+                       torch.empty(B, dtype=torch.int32, device=DEV), torch.empty(B, dtype=torch.int32, device=DEV))
+                for _ in range(20):
+                    f.fann_build_lut(ix.handle, q, B, cb, w.cfg.dsub, lut, st.cuda_stream)
+                    f.fann_dedup_scan_topk(ix.handle, lut, B, off, ids, total, k, out[0], out[1], out[2], out[3],
+                                           ws, need, st.cuda_stream)
+                f.fann_workspace_status(ix.handle, ws, st.cuda_stream)
+                st.synchronize()
+                results[t] = (np_u32(out[0]), out[1].cpu().numpy(), np_u32(out[2]), np_u32(out[3]))
+        except Exception as e:                                 # noqa: BLE001
+            errors.append(e)
+
+    th = [threading.Thread(target=worker, args=(t,)) for t in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not errors, errors
+    for t in range(2):
+        for a, b in zip(results[t], serial):
+            assert np.array_equal(a, b)
+    ix.close()
 
 
 def test_load_codes_from_host_and_in_chunks(fann, w_i8):

@@ -3,7 +3,7 @@ import numpy as np
 import torch
 
 from workloads import CONFIGS, DEFAULT_SEED, make_lists, make_probes, make_candidates, mini, make_codebooks, \
-    make_codes, encode_nearest, draw_vectors, stream_key
+    make_codes, encode_nearest, draw_vectors, stream_key, feistel_permute
 
 
 def test_tiny_shapes_and_ranges(tiny_local):
@@ -75,3 +75,20 @@ def test_integer_configs_stay_integer():
         cb = make_codebooks(cfg, DEFAULT_SEED)
         assert torch.equal(cb, cb.round())
         assert cfg.M * cfg.dsub * 255 ** 2 < 2 ** 24             # every ADC sum exact in fp32
+
+
+def test_feistel_id_map_is_a_bijection_that_scatters():
+    """the vector -> ID map is a seeded random bijection of [0, N), not a lattice."""
+    for N in (1000, 100_003, 1 << 16, (1 << 16) + 1):
+        y = feistel_permute(torch.arange(N, dtype=torch.int64), N, key=99).numpy()
+        assert y.min() == 0 and y.max() == N - 1 and np.unique(y).size == N
+    N = 1_000_000_000                                            # config 4/5 size, a window of consecutive t
+    t = torch.arange(5_000_000, 5_200_000, dtype=torch.int64)
+    y = np.sort(feistel_permute(t, N, key=7).numpy())
+    assert y.min() >= 0 and y.max() < N and np.unique(y).size == t.numel()
+    gaps = np.diff(y).astype(np.float64)
+    # uniformly random positions have exponential gaps (cv = 1); a Kronecker lattice has three gap lengths (cv << 1)
+    assert 0.9 < gaps.std() / gaps.mean() < 1.1
+    assert np.unique(gaps).size > 1000
+    y2 = feistel_permute(t, N, key=8).numpy()
+    assert not np.array_equal(np.sort(y2), y)                    # keyed

@@ -33,6 +33,7 @@ class WorkloadConfig:
     window_factor: int     # window = window_factor * nprobe lists around a centre
     codes_mode: str        # 'encode' (true nearest-centroid) | 'histogram'
     integer_exact: bool    # all fp32 arithmetic exact (integers < 2^24)
+    id_map: str = "feistel"  # distinct vector -> ID: 'feistel' (seeded random bijection of [0, N)) | 'lattice' ((A t + c) mod N)
 
     @property
     def dsub(self) -> int:

@@ -182,6 +182,53 @@ def make_codes(cfg: WorkloadConfig, seed: int, codebooks: torch.Tensor,
 
 
 # --------------------------------------------------------------------------
+# vector -> ID maps
+# --------------------------------------------------------------------------
+
+_FEISTEL_ROUNDS = 4
+
+
+def feistel_permute(x: torch.Tensor, N: int, key: int) -> torch.Tensor:
+    """Seeded bijection of [0, N) (int64 in, int64 out): a 4-round unbalanced Feistel network on
+    ceil(log2 N) bits -- round i xors one half with a hash of the other half, so every round is
+    invertible -- with cycle-walking: a value that lands in [N, 2^bits) goes through the network
+    again until it falls below N.  A list's IDs then behave like uniformly random distinct
+    positions of the code array (SURVEY.md 8(d) "Vector -> ID")."""
+    bits = max(2, (N - 1).bit_length())
+    a = bits // 2                      # low half
+    b = bits - a                       # high half
+    ma, mb = (1 << a) - 1, (1 << b) - 1
+    keys = [stream_key(key, "feistel", r) for r in range(_FEISTEL_ROUNDS)]
+
+    def network(v):
+        lo, hi = v & ma, (v >> a) & mb
+        for r in range(_FEISTEL_ROUNDS):
+            if r % 2 == 0:
+                hi = hi ^ (_lsr(hash64(keys[r], lo), 20) & mb)
+            else:
+                lo = lo ^ (_lsr(hash64(keys[r], hi), 20) & ma)
+        return (hi << a) | lo
+
+    y = network(x)
+    while True:
+        out = y >= N
+        if not bool(out.any()):
+            return y
+        y = torch.where(out, network(y), y)
+
+
+def vector_ids(cfg: WorkloadConfig, seed: int, t: torch.Tensor) -> torch.Tensor:
+    """IDs (int64) of the distinct vectors with indices t (int64, < N)."""
+    if cfg.id_map == "lattice":
+        # Kronecker lattice: very evenly spread (three gap lengths) -- the friendliest case for an
+        # order-preserving dedup table; kept for A/B measurements only
+        return (t * _ID_MULT + stream_key(seed, cfg.name, "id_add") % cfg.N) % cfg.N
+    if cfg.id_map == "feistel":
+        return feistel_permute(t, cfg.N, stream_key(seed, cfg.name, "id_map"))
+    raise ValueError(cfg.id_map)
+
+
+# --------------------------------------------------------------------------
 # posting lists with boundary replication
 # --------------------------------------------------------------------------
 
@@ -266,7 +313,6 @@ def make_lists(cfg: WorkloadConfig, seed: int, device="cpu",
     assert T <= N, f"{T} distinct vectors > N={N}"
     krep = stream_key(seed, cfg.name, "replicas")
     srcs = _sources(cfg)
-    id_add = stream_key(seed, cfg.name, "id_add") % N
 
     def chunk_attrs(l0, l1):
         t0, t1 = int(home_start[l0]), int(home_start[l1])
@@ -296,7 +342,7 @@ def make_lists(cfg: WorkloadConfig, seed: int, device="cpu",
     for l0 in range(0, L, lists_per_chunk):
         l1 = min(L, l0 + lists_per_chunk)
         t, home, r, sigma = chunk_attrs(l0, l1)
-        vid = ((t * _ID_MULT + id_add) % N).to(torch.int32)
+        vid = vector_ids(cfg, seed, t).to(torch.int32)
         for si, delta in enumerate(srcs):
             mask = _has_offset(r, sigma, delta)
             idx = torch.nonzero(mask, as_tuple=False).squeeze(1)
