@@ -49,6 +49,13 @@ def _load():
                                          p, C.c_uint64, p, p]
         lib.oracle_query_all.restype = C.c_uint64
         lib.oracle_max_threads.restype = C.c_int
+        lib.oracle_expand_lists.argtypes = [p, p, C.c_uint64, p, C.c_uint32, C.c_uint32, p, p]
+        lib.oracle_expand_lists.restype = C.c_uint64
+        lib.oracle_rerank.argtypes = [p, p, C.c_uint64, C.c_uint32, p, C.c_uint32, C.c_uint32, C.c_uint32,
+                                      C.c_float, C.c_uint32, p, p, p, p, p]
+        lib.oracle_rerank.restype = C.c_uint32
+        lib.oracle_page_reads.argtypes = [p, C.c_uint64, p, C.c_uint32, C.c_uint32, C.c_uint32, p, C.c_uint64, p, p]
+        lib.oracle_page_reads.restype = C.c_uint32
         _lib = lib
     return _lib
 
@@ -142,3 +149,73 @@ def query_all(query, codebooks, codes, ids, N=None):
     u = _load().oracle_query_all(_ptr(q), _ptr(cb), _ptr(cd), int(N), M, dsub, _ptr(a), a.size,
                                  _ptr(ai), _ptr(ad))
     return ai[:u].copy(), ad[:u].copy()
+
+
+def expand_lists(list_offsets, list_ids, probes):
+    """PAPER.md:L125 step (3): probes [B, nprobe] u32 (list indices) -> (cand_offsets [B+1] i64, cand_ids u32),
+    each query's candidates = its probed lists' IDs concatenated in probe order."""
+    lo = _arr(list_offsets, np.int64)
+    li = _arr(np.asarray(list_ids).view(np.uint32) if np.asarray(list_ids).dtype == np.int32 else list_ids, np.uint32)
+    pr = np.asarray(probes)
+    pr = _arr(pr.view(np.uint32) if pr.dtype == np.int32 else pr, np.uint32)
+    B, nprobe = pr.shape
+    off = np.empty(B + 1, dtype=np.int64)
+    total = _load().oracle_expand_lists(_ptr(lo), _ptr(li), lo.size - 1, _ptr(pr), B, nprobe, _ptr(off), None)
+    ids = np.empty(max(1, total), dtype=np.uint32)
+    _load().oracle_expand_lists(_ptr(lo), _ptr(li), lo.size - 1, _ptr(pr), B, nprobe, _ptr(off), _ptr(ids))
+    return off, ids[:total]
+
+
+def search_lists(queries, codebooks, codes, list_offsets, list_ids, probes, k, N=None, nthreads=0):
+    """Steps (3)(1)(5)(6)(7): expand the probed lists, then the whole GPU stage on the CPU."""
+    off, ids = expand_lists(list_offsets, list_ids, probes)
+    return search(queries, codebooks, codes, off, ids, k, N=N, nthreads=nthreads)
+
+
+def rerank(queries, vectors, tasks, batch_size, k, eps, beta):
+    """Algorithm 1 for every query.  queries [B, d] f32, vectors [N, d] f32 raw vectors,
+    tasks [B, n] u32 candidate IDs in ascending PQ order (0xFFFFFFFF padded).  Returns a dict: ids [B,k] u32,
+    dists [B,k] f32, dists64 [B,k] f64, counts [B], batches [B] (mini-batches executed), reads [B] (vectors read)."""
+    q = _arr(queries, np.float32)
+    v = _arr(vectors, np.float32)
+    t = np.asarray(tasks)
+    t = _arr(t.view(np.uint32) if t.dtype == np.int32 else t, np.uint32)
+    B, n = t.shape
+    N, d = v.shape
+    assert q.shape == (B, d)
+    oi = np.empty((B, k), dtype=np.uint32)
+    od = np.empty((B, k), dtype=np.float32)
+    od64 = np.empty((B, k), dtype=np.float64)
+    cnt = np.zeros(B, dtype=np.uint32)
+    bat = np.zeros(B, dtype=np.uint32)
+    reads = np.zeros(B, dtype=np.uint32)
+    lib = _load()
+    for b in range(B):
+        c, nb = C.c_uint32(0), C.c_uint32(0)
+        reads[b] = lib.oracle_rerank(_ptr(q[b]), _ptr(v), N, d, _ptr(t[b]), n, batch_size, k, eps, beta,
+                                     _ptr(oi[b]), _ptr(od[b]), _ptr(od64[b]), C.byref(c), C.byref(nb))
+        cnt[b], bat[b] = c.value, nb.value
+    return {"ids": oi, "dists": od, "dists64": od64, "counts": cnt, "batches": bat, "reads": reads}
+
+
+def page_reads(page_of, tasks, batch_size, max_batches=None, resident=None, n_pages=0):
+    """Fig. 8 for every query.  page_of [N] u32, tasks [B, n] u32, max_batches [B] or None,
+    resident: uint32 bitmap over pages or None.  Returns (pages [B, n] u32 padded with 0xFFFFFFFF,
+    batch_reads [B, nb] u32, total [B] u32)."""
+    po = _arr(page_of, np.uint32)
+    t = np.asarray(tasks)
+    t = _arr(t.view(np.uint32) if t.dtype == np.int32 else t, np.uint32)
+    B, n = t.shape
+    nb = (n + batch_size - 1) // batch_size
+    pages = np.full((B, n), ID_NONE, dtype=np.uint32)
+    br = np.zeros((B, nb), dtype=np.uint32)
+    tot = np.zeros(B, dtype=np.uint32)
+    res = None if resident is None else _arr(resident, np.uint32)
+    lib = _load()
+    for b in range(B):
+        mb = 0 if max_batches is None else int(max_batches[b])
+        row = np.empty(n, dtype=np.uint32)
+        tot[b] = lib.oracle_page_reads(_ptr(po), po.size, _ptr(t[b]), n, batch_size, mb,
+                                       None if res is None else _ptr(res), n_pages, _ptr(row), _ptr(br[b]))
+        pages[b, :tot[b]] = row[:tot[b]]
+    return pages, br, tot

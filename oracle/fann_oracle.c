@@ -13,6 +13,10 @@
  *   (5) vector-ID dedup         PAPER.md:L127       -> oracle_dedup
  *   (6) PQ (ADC) distance       PAPER.md:L84 Eq. 1  -> oracle_adc
  *   (7) sort, return top-n      PAPER.md:L133       -> oracle_topk
+ * and the rows SURVEY.md 8(f) adds around that path:
+ *   (3) list metadata -> candidate IDs   PAPER.md:L125, L150   -> oracle_expand_lists   (NEXT-2)
+ *   (8) heuristic re-ranking, Alg. 1     PAPER.md:L164-L182    -> oracle_rerank         (NEXT-1)
+ *       page-level I/O dedup, Fig. 8     PAPER.md:L198         -> oracle_page_reads     (NEXT-4)
  *
  * The method reaches exactly a plainly-defined result (set of distinct IDs, a
  * finite sum, the k smallest), so each function below IS that definition:
@@ -188,6 +192,190 @@ uint64_t oracle_query_all(const float *q, const float *codebooks, const uint8_t 
 {
     return one_query(q, codebooks, codes, N, M, dsub, ids, C, 0, NULL, NULL, NULL, NULL,
                      all_ids, all_d64);
+}
+
+/* NEXT-2, PAPER.md:L125 step (3) "the CPU ... consults the metadata to obtain the vector-IDs
+ * in these posting lists" (L150: the metadata holds only the vector-IDs of every list): the candidate list of a
+ * query is the concatenation, in probe order, of the ID arrays of the posting lists it probes.  Readings
+ * (R21): a probe equal to 0xFFFFFFFF is padding and a probe >= n_lists names no list; both contribute
+ * nothing.  Two-pass use: with cand_ids == NULL only cand_offsets[B+1] is written; returns the total. */
+uint64_t oracle_expand_lists(const int64_t *list_offsets, const uint32_t *list_ids, uint64_t n_lists,
+                             const uint32_t *probes, uint32_t B, uint32_t nprobe,
+                             int64_t *cand_offsets, uint32_t *cand_ids)
+{
+    uint64_t total = 0;
+    for (uint32_t b = 0; b < B; ++b) {
+        cand_offsets[b] = (int64_t)total;
+        for (uint32_t j = 0; j < nprobe; ++j) {
+            uint32_t l = probes[(size_t)b * nprobe + j];
+            if (l == ORACLE_ID_NONE || (uint64_t)l >= n_lists) continue;
+            for (int64_t e = list_offsets[l]; e < list_offsets[l + 1]; ++e) {
+                if (cand_ids) cand_ids[total] = list_ids[e];
+                ++total;
+            }
+        }
+    }
+    cand_offsets[B] = (int64_t)total;
+    return total;
+}
+
+/* ---------------------------------------------------------------------------------------------------------
+ * NEXT-1: heuristic re-ranking, PAPER.md:L164-L182 (section 4.2, Eq. 3 at L174, Algorithm 1
+ * at L182).  An iteration with a heuristic stop, so it is followed step by step in the paper's order and
+ * notation: a max-heap Q of capacity k, mini-batches of BatchSize tasks, change rate Delta, StabilityCounter.
+ *
+ * Readings (R22-R25; S20 of SURVEY.md): distance = exact squared L2 on the raw vectors (R1), computed
+ * in fp64 and rounded once to fp32 before any comparison (the precision the GPU decides in); Delta's
+ * denominator is k (Eq. 3; the pseudo-code's "L" is a garbled k); stop when StabilityCounter >= beta
+ * (pseudo-code, L182); "insert ... if its distance is less than the current maximum distance" (L172) is a strict
+ * "<" on the distance, and while Q holds fewer than k vectors every task is inserted; the vector that leaves Q
+ * is the one with the largest distance, the latest inserted among equals (so Q is at all times the k smallest
+ * of the tasks seen so far under the order (distance, position in Tasks)); a task ID equal to 0xFFFFFFFF ends
+ * the task list (padding of the top-n list) and an ID >= N is skipped; Q is returned ascending by
+ * (distance, position).  Delta < eps is evaluated as (double)c / (double)k < (double)eps.
+ * --------------------------------------------------------------------------------------------------------- */
+typedef struct { float d; uint32_t pos; uint32_t id; double d64; } heap_item_t;
+
+static int heap_less(const heap_item_t *a, const heap_item_t *b)        /* order (distance, position) */
+{
+    if (a->d != b->d) return a->d < b->d;
+    return a->pos < b->pos;
+}
+
+static void heap_sift_up(heap_item_t *h, uint32_t i)
+{
+    while (i > 0) {
+        uint32_t p = (i - 1) / 2;
+        if (!heap_less(&h[p], &h[i])) break;
+        heap_item_t t = h[p]; h[p] = h[i]; h[i] = t;
+        i = p;
+    }
+}
+
+static void heap_sift_down(heap_item_t *h, uint32_t n, uint32_t i)
+{
+    for (;;) {
+        uint32_t l = 2 * i + 1, r = l + 1, m = i;
+        if (l < n && heap_less(&h[m], &h[l])) m = l;
+        if (r < n && heap_less(&h[m], &h[r])) m = r;
+        if (m == i) break;
+        heap_item_t t = h[m]; h[m] = h[i]; h[i] = t;
+        i = m;
+    }
+}
+
+static int cmp_heap_item(const void *a, const void *b)
+{
+    const heap_item_t *x = (const heap_item_t *)a, *y = (const heap_item_t *)b;
+    if (heap_less(x, y)) return -1;
+    if (heap_less(y, x)) return 1;
+    return 0;
+}
+
+/* GetDistance(Tasks[j]) of Algorithm 1 line 6, without the SSD: exact squared L2 in fp64. */
+static double exact_dist(const float *q, const float *v, uint32_t d)
+{
+    double s = 0.0;
+    for (uint32_t t = 0; t < d; ++t) {
+        double delta = (double)q[t] - (double)v[t];
+        s += delta * delta;
+    }
+    return s;
+}
+
+/* Algorithm 1 for one query.  tasks[n]: candidate IDs in ascending PQ-distance order (the GPU stage's top-n,
+ * L170).  Writes Q ascending into out_ids/out_dists[k] (padded with 0xFFFFFFFF / +inf), *out_count = |Q|,
+ * *out_batches = mini-batches executed.  Returns the number of tasks whose raw vector was read. */
+uint32_t oracle_rerank(const float *query, const float *vectors, uint64_t N, uint32_t d,
+                       const uint32_t *tasks, uint32_t n, uint32_t batch_size, uint32_t k,
+                       float eps, uint32_t beta,
+                       uint32_t *out_ids, float *out_dists, double *out_dists64,
+                       uint32_t *out_count, uint32_t *out_batches)
+{
+    heap_item_t *Q = (heap_item_t *)malloc((size_t)(k ? k : 1) * sizeof(heap_item_t));   /* line 1: Q <- NULL */
+    uint32_t *S_prev = (uint32_t *)malloc((size_t)(k ? k : 1) * sizeof(uint32_t));
+    uint32_t qn = 0, stability = 0, batches = 0, reads = 0;                               /* line 2 */
+    uint32_t n_tasks = 0;
+    while (n_tasks < n && tasks[n_tasks] != ORACLE_ID_NONE) ++n_tasks;                    /* padding ends the list */
+    int done = 0;
+    for (uint32_t i = 0; i < n_tasks && !done; i += batch_size) {                         /* line 3 */
+        uint32_t prev_n = qn;
+        for (uint32_t s = 0; s < qn; ++s) S_prev[s] = Q[s].id;                            /* line 4: S_{n-1} */
+        for (uint32_t j = i; j < i + batch_size && j < n_tasks; ++j) {                    /* line 5 */
+            uint32_t id = tasks[j];
+            if ((uint64_t)id >= N) continue;
+            double d64 = exact_dist(query, vectors + (size_t)id * d, d);                  /* line 6 */
+            ++reads;
+            heap_item_t c; c.d = (float)d64; c.pos = j; c.id = id; c.d64 = d64;
+            if (qn < k) {                                                                 /* line 7: Q.insert */
+                Q[qn] = c; heap_sift_up(Q, qn); ++qn;
+            } else if (k > 0 && c.d < Q[0].d) {
+                Q[0] = c; heap_sift_down(Q, qn, 0);
+            }
+        }
+        ++batches;
+        uint32_t changed = 0;                                                             /* lines 9-10: Delta */
+        for (uint32_t s = 0; s < qn; ++s) {
+            int in_prev = 0;
+            for (uint32_t t = 0; t < prev_n; ++t) if (S_prev[t] == Q[s].id) { in_prev = 1; break; }
+            if (!in_prev) ++changed;
+        }
+        double delta = (double)changed / (double)k;
+        if (delta < (double)eps) {                                                        /* line 11 */
+            ++stability;                                                                  /* line 12 */
+            if (stability >= beta) done = 1;                                              /* lines 13-14 */
+        } else {
+            stability = 0;                                                                /* line 17 */
+        }
+    }
+    qsort(Q, qn, sizeof(heap_item_t), cmp_heap_item);                                     /* line 20: return Q */
+    for (uint32_t s = 0; s < k; ++s) {
+        if (s < qn) {
+            out_ids[s] = Q[s].id; out_dists[s] = Q[s].d;
+            if (out_dists64) out_dists64[s] = Q[s].d64;
+        } else {
+            out_ids[s] = ORACLE_ID_NONE; out_dists[s] = INFINITY;
+            if (out_dists64) out_dists64[s] = INFINITY;
+        }
+    }
+    *out_count = qn;
+    *out_batches = batches;
+    free(Q); free(S_prev);
+    return reads;
+}
+
+/* ---------------------------------------------------------------------------------------------------------
+ * NEXT-4: redundancy-aware I/O deduplication, PAPER.md:L198 (section 4.3, Fig. 8).
+ * "merging I/Os mapped to the same SSD page within a mini-batch, and exploiting the DRAM buffer to eliminate
+ * redundant I/Os in subsequent mini-batches".  For one query: the mapping table gives the page of each task's
+ * vector; a mini-batch reads each page it needs once, unless the DRAM buffer already holds it; pages read
+ * enter the buffer.
+ *
+ * Readings (R26): the buffer is per query, unbounded, and starts with the pages whose bit is set in
+ * `resident` (may be NULL = empty); a task equal to 0xFFFFFFFF ends the list, an ID >= N is skipped; the
+ * pages of a mini-batch are reported in order of first need.  Only the first `max_batches` mini-batches are
+ * processed (what Algorithm 1 executed); 0 = all.
+ * page_of[N]; out_pages[n] receives the pages read, mini-batch after mini-batch; out_batch_reads[nb] the number
+ * of page reads (I/Os) of each mini-batch, nb = ceil(n / batch_size).  Returns the total number of reads.
+ * --------------------------------------------------------------------------------------------------------- */
+uint32_t oracle_page_reads(const uint32_t *page_of, uint64_t N, const uint32_t *tasks, uint32_t n,
+                           uint32_t batch_size, uint32_t max_batches, const uint32_t *resident, uint64_t n_pages,
+                           uint32_t *out_pages, uint32_t *out_batch_reads)
+{
+    uint32_t n_tasks = 0, total = 0, nb = (n + batch_size - 1) / batch_size;
+    while (n_tasks < n && tasks[n_tasks] != ORACLE_ID_NONE) ++n_tasks;
+    for (uint32_t t = 0; t < nb; ++t) out_batch_reads[t] = 0;
+    for (uint32_t i = 0, t = 0; i < n_tasks; i += batch_size, ++t) {
+        if (max_batches && t >= max_batches) break;
+        for (uint32_t j = i; j < i + batch_size && j < n_tasks; ++j) {
+            if ((uint64_t)tasks[j] >= N) continue;
+            uint32_t p = page_of[tasks[j]];
+            int have = resident && (uint64_t)p < n_pages && ((resident[p >> 5] >> (p & 31)) & 1u);
+            for (uint32_t s = 0; s < total && !have; ++s) if (out_pages[s] == p) have = 1;   /* buffer + this batch */
+            if (!have) { out_pages[total++] = p; ++out_batch_reads[t]; }
+        }
+    }
+    return total;
 }
 
 int oracle_max_threads(void)
