@@ -62,6 +62,8 @@ enum {
 #define FANN_ID_NONE 0xFFFFFFFFu               /* padding in candidate lists and in outputs */
 #define FANN_MAX_M   64u                       /* PQ bytes per vector (lookup table <= 64 KB) */
 #define FANN_MAX_K   1024u                     /* candidates returned per query             */
+#define FANN_MAX_NPROBE 8192u                  /* posting lists probed per query (fann_search_lists) */
+enum { FANN_ELEM_F32 = 0, FANN_ELEM_U8 = 1, FANN_ELEM_I8 = 2 };   /* raw-vector element types (fann_load_vectors) */
 
 /* Create an index on CUDA device `device`.  *out receives the handle. */
 int  fann_create(fann_index **out, int device);
@@ -186,6 +188,125 @@ int fann_search_host(fann_index *ix, const float *queries_h, uint32_t B,
                      const int64_t *cand_offsets_h, const uint32_t *cand_ids_h,
                      uint32_t k, uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h,
                      void *device_scratch, size_t scratch_bytes, void *stream);
+
+/* ======================================================================================
+ * Steps around the hot path.  Each is optional: the calls above never need
+ * them.
+ * ====================================================================================== */
+
+/*
+ * NEXT-2 -- posting-list metadata resident in HBM.  PAPER.md:L150: the host keeps, per posting
+ * list, only its vector-IDs; L125 steps (3)(4): the CPU concatenates the IDs of the top-m lists
+ * and sends them to the GPU -- 5 GB per batch at the largest configuration, 4x the time of the
+ * kernels over PCIe.  On a 180 GB part the ID arrays of all lists (4 bytes per list entry) fit
+ * beside the codes, so the host sends nprobe list indices per query instead and step (3) runs
+ * on the GPU.
+ *
+ * fann_load_lists copies the CSR of all posting lists into library-owned HBM (replacing any
+ * earlier lists): list l holds list_ids[list_offsets[l] .. list_offsets[l+1]).
+ * list_offsets  [n_lists + 1] int64, list_offsets[0] == 0, list_offsets[n_lists] == n_entries
+ * list_ids      [n_entries] uint32 vector-IDs (any order inside a list)
+ * Host or device source (src_is_device); synchronises `stream`.
+ * Errors: EINVAL (NULL, n_lists == 0, offsets do not end at n_entries), ENOMEM, ECUDA.
+ */
+int fann_load_lists(fann_index *ix, const int64_t *list_offsets, const uint32_t *list_ids,
+                    uint64_t n_lists, uint64_t n_entries, int src_is_device, void *stream);
+
+/*
+ * Steps (3)(5)(6)(7) from probed list indices.  Query b's candidate list is the concatenation,
+ * in probe order, of the ID arrays of lists probes[b][0 .. nprobe); a probe equal to
+ * FANN_ID_NONE is padding and a probe >= n_lists names no list -- both contribute nothing.
+ * From there the call is fann_dedup_scan_topk on those lists: same kernels, same results.
+ * probes           device, [B][nprobe] uint32
+ * max_total_cands  capacity the workspace is sized for: an upper bound of the batch's total
+ *                  candidate count (sum of the probed lists' lengths).  If the batch needs
+ *                  more, nothing is scored and fann_search_lists_status returns
+ *                  FANN_EWORKSPACE together with the count that would have been needed.
+ * workspace        device, >= fann_search_lists_workspace_bytes(ix, B, max_total_cands, k)
+ * lut, out_*       as in fann_dedup_scan_topk.  Enqueues only.
+ * fann_search_lists_status synchronises `stream` and returns FANN_OK, FANN_EWORKSPACE (see
+ * above) or what fann_workspace_status would; *total_cands (may be NULL) receives the batch's
+ * candidate count.  B, max_total_cands and k must repeat the values of the call.
+ */
+size_t fann_search_lists_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t max_total_cands, uint32_t k);
+int fann_search_lists(fann_index *ix, const float *lut, uint32_t B,
+                      const uint32_t *probes, uint32_t nprobe, uint64_t max_total_cands, uint32_t k,
+                      uint32_t *out_ids, float *out_dists, uint32_t *out_counts, uint32_t *out_uniq,
+                      void *workspace, size_t workspace_bytes, void *stream);
+int fann_search_lists_status(fann_index *ix, const void *workspace, uint32_t B, uint64_t max_total_cands,
+                             uint32_t k, uint64_t *total_cands, void *stream);
+
+/*
+ * The same from HOST buffers: query vectors and probes go up (B * (4 d + 4 nprobe) bytes),
+ * ids / dists / counts come back; synchronises `stream` and returns the batch's status.
+ * queries_h, probes_h, out_*_h: host pointers (pinned memory gives asynchronous copies).
+ */
+size_t fann_search_lists_host_scratch_bytes(const fann_index *ix, uint32_t B, uint32_t dsub, uint32_t nprobe,
+                                            uint64_t max_total_cands, uint32_t k);
+int fann_search_lists_host(fann_index *ix, const float *queries_h, uint32_t B,
+                           const float *codebooks_d, uint32_t dsub,
+                           const uint32_t *probes_h, uint32_t nprobe, uint64_t max_total_cands, uint32_t k,
+                           uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h,
+                           void *device_scratch, size_t scratch_bytes, void *stream);
+
+/*
+ * NEXT-1 -- heuristic re-ranking, PAPER.md:L164-L182 (section 4.2, Eq. 3, Algorithm 1), with the
+ * raw vectors in HBM instead of on SSD (the configurations whose raw vectors fit).
+ *
+ * fann_load_vectors copies rows [first, first + n) of the N_total x d raw-vector array
+ * (row-major, elem_type FANN_ELEM_F32 / _U8 / _I8, `vectors` points at row `first`) into
+ * library-owned HBM; the first call fixes (N_total, d, elem_type).  d <= 2048.
+ *
+ * fann_rerank runs Algorithm 1 for B queries.  task_ids[b][0 .. n) is the query's candidate
+ * list in ascending PQ-distance order -- out_ids of the calls above (L170) -- ended by
+ * FANN_ID_NONE padding; an ID >= N_total is skipped.  Mini-batches of batch_size tasks are
+ * executed in order: exact squared L2 distance (fp32) to the raw vector of every task, the
+ * vector enters Q if Q holds fewer than k vectors or its distance is less than Q's largest
+ * (the vector with the largest distance, the latest inserted among equals, leaves);
+ * Delta = |S_n - S_n n S_{n-1}| / k (Eq. 3); the StabilityCounter counts consecutive
+ * mini-batches with Delta < eps and the query stops when it reaches beta.  Raw vectors of
+ * mini-batches after the stop are not read.
+ * queries      device, [B][d] fp32           task_ids  device, [B][n] uint32, n <= 2048
+ * out_ids      device, [B][k] uint32: Q ascending by (distance, position in task_ids), padded
+ *              with FANN_ID_NONE;  out_dists [B][k] fp32, padded with +inf;  k <= 1024
+ * out_counts   device, [B]: |Q|
+ * out_batches  device, [B]: mini-batches executed (may be NULL)
+ * out_reads    device, [B]: raw vectors read (may be NULL)
+ * batch_size > n is taken as n.  Enqueues only; needs no workspace.
+ * Errors: EINVAL (NULL, zero sizes, beta == 0, eps < 0, vectors not loaded), EUNSUPPORTED.
+ */
+int fann_load_vectors(fann_index *ix, const void *vectors, uint64_t first, uint64_t n, uint64_t N_total,
+                      uint32_t d, int elem_type, int src_is_device, void *stream);
+int fann_rerank(fann_index *ix, const float *queries, uint32_t B, const uint32_t *task_ids, uint32_t n,
+                uint32_t batch_size, uint32_t k, float eps, uint32_t beta,
+                uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
+                uint32_t *out_batches, uint32_t *out_reads, void *stream);
+
+/*
+ * NEXT-4 -- page-level I/O deduplication, PAPER.md:L198 (section 4.3, Fig. 8): "merging I/Os
+ * mapped to the same SSD page within a mini-batch, and exploiting the DRAM buffer to eliminate
+ * redundant I/Os in subsequent mini-batches".  The library computes WHICH pages each
+ * mini-batch of each query has to read; it performs no I/O.
+ *
+ * fann_load_page_table: page_of[v] = SSD page holding raw vector v (the in-memory mapping
+ * table of), N entries, page numbers < n_pages.
+ *
+ * fann_page_reads: for query b, mini-batch t covers task_ids[b][t*batch_size .. +batch_size)
+ * (list ended by FANN_ID_NONE; IDs >= N skipped).  A mini-batch reads each page its vectors
+ * need once, unless the query's DRAM buffer holds it; pages read enter the buffer.  The buffer
+ * starts with the pages whose bit is set in resident_bits (bit p of word p / 32; NULL = empty).
+ * Only the first batches_run[b] mini-batches are processed (what fann_rerank executed;
+ * NULL or 0 = all).
+ * out_pages        device, [B][n]: the pages to read, mini-batch after mini-batch (any order
+ *                  inside one), padded with FANN_ID_NONE;  n <= 4096
+ * out_batch_reads  device, [B][ceil(n / batch_size)]: page reads (I/Os) of each mini-batch
+ * out_total        device, [B]: page reads of the query
+ */
+int fann_load_page_table(fann_index *ix, const uint32_t *page_of, uint64_t N, uint64_t n_pages,
+                         int src_is_device, void *stream);
+int fann_page_reads(fann_index *ix, const uint32_t *task_ids, uint32_t B, uint32_t n, uint32_t batch_size,
+                    const uint32_t *batches_run, const uint32_t *resident_bits,
+                    uint32_t *out_pages, uint32_t *out_batch_reads, uint32_t *out_total, void *stream);
 
 /* Geometry and counters, for benchmarks and tests. */
 typedef struct fann_info {

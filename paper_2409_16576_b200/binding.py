@@ -19,6 +19,8 @@ _LIB_PATH = os.path.join(HERE, "libfann.so")
 FANN_ID_NONE = 0xFFFFFFFF
 FANN_MAX_M = 64
 FANN_MAX_K = 1024
+FANN_MAX_NPROBE = 8192
+FANN_ELEM_F32, FANN_ELEM_U8, FANN_ELEM_I8 = 0, 1, 2
 FANN_OK = 0
 
 _lib = None
@@ -66,6 +68,16 @@ def load_library():
         "fann_workspace_status": (i, [p, p, p]),
         "fann_search_host_scratch_bytes": (sz, [p, u32, u32, u64, u32]),
         "fann_search_host": (i, [p, p, u32, p, u32, p, p, u32, p, p, p, p, sz, p]),
+        "fann_load_lists": (i, [p, p, p, u64, u64, i, p]),
+        "fann_search_lists_workspace_bytes": (sz, [p, u32, u64, u32]),
+        "fann_search_lists": (i, [p, p, u32, p, u32, u64, u32, p, p, p, p, p, sz, p]),
+        "fann_search_lists_status": (i, [p, p, u32, u64, u32, C.POINTER(u64), p]),
+        "fann_search_lists_host_scratch_bytes": (sz, [p, u32, u32, u32, u64, u32]),
+        "fann_search_lists_host": (i, [p, p, u32, p, u32, p, u32, u64, u32, p, p, p, p, sz, p]),
+        "fann_load_vectors": (i, [p, p, u64, u64, u64, u32, i, i, p]),
+        "fann_rerank": (i, [p, p, u32, p, u32, u32, u32, C.c_float, u32, p, p, p, p, p, p]),
+        "fann_load_page_table": (i, [p, p, u64, u64, i, p]),
+        "fann_page_reads": (i, [p, p, u32, u32, u32, p, p, p, p, p, p]),
         "fann_get_info": (i, [p, C.POINTER(_Info)]),
         "fann_set_timing": (i, [p, i]),
         "fann_last_timing": (i, [p] + [C.POINTER(C.c_float)] * 4),
@@ -162,6 +174,73 @@ def fann_search_host(ix, queries_h, B, codebooks_d, dsub, cand_offsets_h, cand_i
                                            _addr(cand_offsets_h), _addr(cand_ids_h), k, _addr(out_ids_h),
                                            _addr(out_dists_h), _addr(out_counts_h), _addr(device_scratch),
                                            scratch_bytes, stream))
+
+
+def fann_load_lists(ix, list_offsets, list_ids, n_lists, n_entries, src_is_device, stream=None) -> None:
+    _check(load_library().fann_load_lists(ix, _addr(list_offsets), _addr(list_ids), n_lists, n_entries,
+                                          int(src_is_device), stream))
+
+
+def fann_search_lists_workspace_bytes(ix, B, max_total_cands, k) -> int:
+    n = load_library().fann_search_lists_workspace_bytes(ix, B, max_total_cands, k)
+    if n == 0:
+        raise FannError(-1, fann_last_error())
+    return n
+
+
+def fann_search_lists(ix, lut, B, probes, nprobe, max_total_cands, k, out_ids, out_dists, out_counts, out_uniq,
+                      workspace, workspace_bytes, stream=None) -> None:
+    _check(load_library().fann_search_lists(ix, _addr(lut), B, _addr(probes), nprobe, max_total_cands, k,
+                                            _addr(out_ids), _addr(out_dists), _addr(out_counts), _addr(out_uniq),
+                                            _addr(workspace), workspace_bytes, stream))
+
+
+def fann_search_lists_status(ix, workspace, B, max_total_cands, k, stream=None) -> int:
+    """Raises on a bad status; returns the batch's candidate count."""
+    total = C.c_uint64(0)
+    rc = load_library().fann_search_lists_status(ix, _addr(workspace), B, max_total_cands, k, C.byref(total), stream)
+    if rc != FANN_OK:
+        err = FannError(rc, fann_last_error())
+        err.total_cands = int(total.value)
+        raise err
+    return int(total.value)
+
+
+def fann_search_lists_host_scratch_bytes(ix, B, dsub, nprobe, max_total_cands, k) -> int:
+    n = load_library().fann_search_lists_host_scratch_bytes(ix, B, dsub, nprobe, max_total_cands, k)
+    if n == 0:
+        raise FannError(-1, fann_last_error())
+    return n
+
+
+def fann_search_lists_host(ix, queries_h, B, codebooks_d, dsub, probes_h, nprobe, max_total_cands, k, out_ids_h,
+                           out_dists_h, out_counts_h, device_scratch, scratch_bytes, stream=None) -> None:
+    _check(load_library().fann_search_lists_host(ix, _addr(queries_h), B, _addr(codebooks_d), dsub, _addr(probes_h),
+                                                 nprobe, max_total_cands, k, _addr(out_ids_h), _addr(out_dists_h),
+                                                 _addr(out_counts_h), _addr(device_scratch), scratch_bytes, stream))
+
+
+def fann_load_vectors(ix, vectors, first, n, N_total, d, elem_type, src_is_device, stream=None) -> None:
+    _check(load_library().fann_load_vectors(ix, _addr(vectors), first, n, N_total, d, elem_type,
+                                            int(src_is_device), stream))
+
+
+def fann_rerank(ix, queries, B, task_ids, n, batch_size, k, eps, beta, out_ids, out_dists, out_counts,
+                out_batches=None, out_reads=None, stream=None) -> None:
+    _check(load_library().fann_rerank(ix, _addr(queries), B, _addr(task_ids), n, batch_size, k, float(eps), beta,
+                                      _addr(out_ids), _addr(out_dists), _addr(out_counts), _addr(out_batches),
+                                      _addr(out_reads), stream))
+
+
+def fann_load_page_table(ix, page_of, N, n_pages, src_is_device, stream=None) -> None:
+    _check(load_library().fann_load_page_table(ix, _addr(page_of), N, n_pages, int(src_is_device), stream))
+
+
+def fann_page_reads(ix, task_ids, B, n, batch_size, batches_run, resident_bits, out_pages, out_batch_reads,
+                    out_total, stream=None) -> None:
+    _check(load_library().fann_page_reads(ix, _addr(task_ids), B, n, batch_size, _addr(batches_run),
+                                          _addr(resident_bits), _addr(out_pages), _addr(out_batch_reads),
+                                          _addr(out_total), stream))
 
 
 def fann_get_info(ix) -> dict:
@@ -274,6 +353,68 @@ class FannIndex:
     def search(self, queries, codebooks, cand_offsets, cand_ids, k, check=False):
         lut = self.build_lut(queries, codebooks)
         return self.dedup_scan_topk(lut, cand_offsets, cand_ids, k, check=check)
+
+    def load_lists(self, list_offsets, list_ids):
+        """CSR of all posting lists: int64 [n_lists + 1], int32/uint32 [entries] (torch, cuda or cpu)."""
+        is_dev = bool(getattr(list_offsets, "is_cuda", False))
+        assert bool(getattr(list_ids, "is_cuda", False)) == is_dev
+        fann_load_lists(self.handle, list_offsets, list_ids, list_offsets.numel() - 1, list_ids.numel(), is_dev,
+                        self._stream())
+
+    def search_lists(self, lut, probes, k, max_total_cands, out=None, check=False):
+        """probes: int32 view of uint32 [B, nprobe] on the device.  Returns (ids, dists, counts, uniq)."""
+        torch = self._torch
+        B, nprobe = probes.shape
+        dev = lut.device
+        if out is None:
+            out = (torch.empty((B, k), dtype=torch.int32, device=dev),
+                   torch.empty((B, k), dtype=torch.float32, device=dev),
+                   torch.empty(B, dtype=torch.int32, device=dev),
+                   torch.empty(B, dtype=torch.int32, device=dev))
+        need = fann_search_lists_workspace_bytes(self.handle, B, max_total_cands, k)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = torch.empty(need, dtype=torch.uint8, device=f"cuda:{self.device}")
+        fann_search_lists(self.handle, lut, B, probes, nprobe, max_total_cands, k, out[0], out[1], out[2], out[3],
+                          self._ws, self._ws.numel(), self._stream())
+        if check:
+            fann_search_lists_status(self.handle, self._ws, B, max_total_cands, k, self._stream())
+        return out
+
+    def load_vectors(self, vectors, first: int = 0, N_total: Optional[int] = None):
+        """Raw vectors [n, d]: float32, uint8 or int8 torch tensor (cuda or cpu)."""
+        torch = self._torch
+        n, d = vectors.shape
+        elem = {torch.float32: FANN_ELEM_F32, torch.uint8: FANN_ELEM_U8, torch.int8: FANN_ELEM_I8}[vectors.dtype]
+        assert vectors.is_contiguous()
+        fann_load_vectors(self.handle, vectors, first, n, n if N_total is None else N_total, d, elem,
+                          bool(vectors.is_cuda), self._stream())
+
+    def rerank(self, queries, task_ids, batch_size, k, eps, beta):
+        """Returns (ids [B,k], dists [B,k], counts [B], batches [B], reads [B])."""
+        torch = self._torch
+        B, n = task_ids.shape
+        dev = queries.device
+        out = (torch.empty((B, k), dtype=torch.int32, device=dev), torch.empty((B, k), dtype=torch.float32, device=dev),
+               torch.empty(B, dtype=torch.int32, device=dev), torch.empty(B, dtype=torch.int32, device=dev),
+               torch.empty(B, dtype=torch.int32, device=dev))
+        fann_rerank(self.handle, queries, B, task_ids, n, batch_size, k, eps, beta, *out, stream=self._stream())
+        return out
+
+    def load_page_table(self, page_of, n_pages):
+        fann_load_page_table(self.handle, page_of, page_of.numel(), n_pages, bool(page_of.is_cuda), self._stream())
+
+    def page_reads(self, task_ids, batch_size, batches_run=None, resident_bits=None):
+        """Returns (pages [B,n], batch_reads [B,nb], total [B])."""
+        torch = self._torch
+        B, n = task_ids.shape
+        bs = min(batch_size, n)
+        nb = (n + bs - 1) // bs
+        dev = task_ids.device
+        out = (torch.empty((B, n), dtype=torch.int32, device=dev), torch.empty((B, nb), dtype=torch.int32, device=dev),
+               torch.empty(B, dtype=torch.int32, device=dev))
+        fann_page_reads(self.handle, task_ids, B, n, batch_size, batches_run, resident_bits, *out, stream=self._stream())
+        return out
 
     def info(self) -> dict:
         return fann_get_info(self.handle)

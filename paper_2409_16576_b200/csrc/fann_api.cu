@@ -2,6 +2,7 @@
 // layout, launch geometry, kernel launches.  No compute happens on the host.
 #include "../../include/fann.h"
 #include "fann_kernels.cuh"
+#include "fann_next.cuh"
 
 #include <atomic>
 #include <cstdarg>
@@ -29,6 +30,16 @@ struct fann_index {
     uint8_t *codes = nullptr;              // [N][row_bytes]
     uint8_t *bounce = nullptr;             // staging for host-sourced code chunks
     size_t bounce_bytes = 0;
+    // posting-list metadata, raw vectors and the vector -> page table, each optional
+    long long *list_offsets = nullptr;     // [n_lists + 1]
+    uint32_t *list_ids = nullptr;          // [list_entries]
+    uint64_t n_lists = 0, list_entries = 0;
+    void *vectors = nullptr;               // [vec_N][vec_d] of vec_elem
+    uint64_t vec_N = 0;
+    uint32_t vec_d = 0;
+    int vec_elem = 0;
+    uint32_t *page_of = nullptr;           // [page_N]
+    uint64_t page_N = 0, n_pages = 0;
     int num_sms = 0;
     int smem_optin = 0;                    // max dynamic shared memory per block
     uint32_t chunks = 1;                   // batch chunks (FANN_CHUNKS): partition of chunk i+1 runs beside the scan of chunk i
@@ -231,6 +242,10 @@ extern "C" void fann_destroy(fann_index *ix)
     cudaDeviceSynchronize();
     if (ix->codes) cudaFree(ix->codes);
     if (ix->bounce) cudaFree(ix->bounce);
+    if (ix->list_offsets) cudaFree(ix->list_offsets);
+    if (ix->list_ids) cudaFree(ix->list_ids);
+    if (ix->vectors) cudaFree(ix->vectors);
+    if (ix->page_of) cudaFree(ix->page_of);
     for (CallCtx *c : ix->ctx_pool) destroy_ctx(c);
     for (auto &e : ix->ev_lut) if (e) cudaEventDestroy(e);
     for (auto &e : ix->ev_plan) if (e) cudaEventDestroy(e);
@@ -667,6 +682,299 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
         CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
     CUDA_TRY(cudaStreamSynchronize(stream));
     return fann_workspace_status(ix, s + h.ws, stream);
+}
+
+
+// ---------------------------------------------------------------- NEXT-2: posting lists resident in HBM
+
+extern "C" int fann_load_lists(fann_index *ix, const int64_t *list_offsets, const uint32_t *list_ids,
+                               uint64_t n_lists, uint64_t n_entries, int src_is_device, void *stream_)
+{
+    if (!ix || !list_offsets) return fail(FANN_EINVAL, "fann_load_lists: NULL argument");
+    if (!list_ids && n_entries) return fail(FANN_EINVAL, "fann_load_lists: list_ids is NULL");
+    if (n_lists == 0 || n_lists >= 0xFFFFFFFFull) return fail(FANN_EINVAL, "fann_load_lists: n_lists must be in 1 .. 2^32-2");
+    if (((uintptr_t)list_offsets & 7) != 0 || ((uintptr_t)list_ids & 3) != 0)
+        return fail(FANN_EINVAL, "fann_load_lists: list_offsets must be 8-byte and list_ids 4-byte aligned");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (ix->list_offsets) { cudaFree(ix->list_offsets); ix->list_offsets = nullptr; }
+    if (ix->list_ids) { cudaFree(ix->list_ids); ix->list_ids = nullptr; }
+    ix->n_lists = 0; ix->list_entries = 0;
+    cudaError_t e = cudaMalloc(&ix->list_offsets, (n_lists + 1) * 8);
+    if (e == cudaSuccess) e = cudaMalloc(&ix->list_ids, (n_entries ? n_entries : 1) * 4);
+    if (e != cudaSuccess) {
+        if (ix->list_offsets) { cudaFree(ix->list_offsets); ix->list_offsets = nullptr; }
+        return fail(FANN_ENOMEM, "fann_load_lists: cudaMalloc: %s", cudaGetErrorString(e));
+    }
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CUDA_TRY(cudaMemcpyAsync(ix->list_offsets, list_offsets, (n_lists + 1) * 8, kind, stream));
+    if (n_entries) CUDA_TRY(cudaMemcpyAsync(ix->list_ids, list_ids, n_entries * 4, kind, stream));
+    long long ends[2] = {-1, -1};                              // offsets[0] and offsets[n_lists] bound every read of list_ids
+    CUDA_TRY(cudaMemcpyAsync(&ends[0], ix->list_offsets, 8, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaMemcpyAsync(&ends[1], ix->list_offsets + n_lists, 8, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    if (ends[0] != 0 || ends[1] < 0 || (uint64_t)ends[1] != n_entries) {
+        cudaFree(ix->list_offsets); cudaFree(ix->list_ids);
+        ix->list_offsets = nullptr; ix->list_ids = nullptr;
+        return fail(FANN_EINVAL, "fann_load_lists: list_offsets[0] = %lld, list_offsets[n_lists] = %lld, n_entries = %llu",
+                    ends[0], ends[1], (unsigned long long)n_entries);
+    }
+    ix->n_lists = n_lists; ix->list_entries = n_entries;
+    return FANN_OK;
+}
+
+struct ListsLayout { size_t hdr, offsets, ids, ws, ws_bytes, total; };
+
+static void lists_layout(const fann_index *ix, uint32_t B, uint64_t cap, uint32_t k, ListsLayout *l)
+{
+    Geom g;
+    geometry(ix, k, B, cap, &g);
+    WsLayout w;
+    ws_layout(B, cap, g, true, &w);
+    size_t o = 0;
+    l->hdr = o;     o = align_up(o + sizeof(ListsHeader), 256);
+    l->offsets = o; o = align_up(o + ((size_t)B + 1) * 8, 256);
+    l->ids = o;     o = align_up(o + (size_t)cap * 4 + 16, 256);
+    l->ws = o;      l->ws_bytes = w.total; o += w.total;
+    l->total = o;
+}
+
+extern "C" size_t fann_search_lists_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t max_total_cands, uint32_t k)
+{
+    if (!ix || !ix->codes) { fail(FANN_EINVAL, "fann_search_lists_workspace_bytes: index has no codes"); return 0; }
+    if (B == 0 || k == 0 || k > FANN_MAX_K) { fail(FANN_EINVAL, "fann_search_lists_workspace_bytes: B=%u k=%u", B, k); return 0; }
+    ListsLayout l;
+    lists_layout(ix, B, max_total_cands, k, &l);
+    return l.total;
+}
+
+extern "C" int fann_search_lists(fann_index *ix, const float *lut, uint32_t B, const uint32_t *probes, uint32_t nprobe,
+                                 uint64_t max_total_cands, uint32_t k, uint32_t *out_ids, float *out_dists,
+                                 uint32_t *out_counts, uint32_t *out_uniq, void *workspace, size_t workspace_bytes,
+                                 void *stream_)
+{
+    if (!ix || !lut || !probes || !out_ids || !out_dists) return fail(FANN_EINVAL, "fann_search_lists: NULL argument");
+    if (!ix->codes) return fail(FANN_EINVAL, "fann_search_lists: load codes first");
+    if (!ix->list_offsets) return fail(FANN_EINVAL, "fann_search_lists: load the posting lists first (fann_load_lists)");
+    if (B == 0 || nprobe == 0) return fail(FANN_EINVAL, "fann_search_lists: B or nprobe is 0");
+    if (nprobe > FANN_MAX_NPROBE) return fail(FANN_EUNSUPPORTED, "fann_search_lists: nprobe=%u > %u", nprobe, FANN_MAX_NPROBE);
+    if (k == 0 || k > FANN_MAX_K) return fail(FANN_EUNSUPPORTED, "fann_search_lists: k=%u not in 1..%u", k, FANN_MAX_K);
+    if (((uintptr_t)probes & 3) != 0) return fail(FANN_EINVAL, "fann_search_lists: probes must be 4-byte aligned");
+    ListsLayout l;
+    lists_layout(ix, B, max_total_cands, k, &l);
+    if (!workspace || ((uintptr_t)workspace & 255) != 0) return fail(FANN_EWORKSPACE, "workspace is NULL or not 256-byte aligned");
+    if (workspace_bytes < l.total) return fail(FANN_EWORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, l.total);
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    char *ws = (char *)workspace;
+    ListsHeader *hdr = (ListsHeader *)(ws + l.hdr);
+    long long *offsets = (long long *)(ws + l.offsets);
+    uint32_t *ids = (uint32_t *)(ws + l.ids);
+    lists_count_kernel<<<(B + 7) / 8, 256, 0, stream>>>(ix->list_offsets, ix->n_lists, probes, B, nprobe,
+                                                         (unsigned long long *)offsets);
+    lists_scan_kernel<<<1, 1024, 0, stream>>>((const unsigned long long *)offsets, B, offsets, hdr,
+                                              (unsigned long long)max_total_cands);
+    lists_expand_kernel<<<B, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(ix->list_offsets, ix->list_ids, ix->n_lists,
+                                                                                probes, nprobe, offsets, ids, hdr);
+    ix->launches += 3;
+    CUDA_TRY(cudaGetLastError());
+    // a batch larger than the workspace was sized for leaves cand_offsets[B] > max_total_cands: the path refuses it
+    return run_path(ix, false, lut, B, (const int64_t *)offsets, ids, max_total_cands, k, out_ids, out_dists, out_counts,
+                    out_uniq, nullptr, nullptr, ws + l.ws, l.ws_bytes, stream, 0, false, false);
+}
+
+extern "C" int fann_search_lists_status(fann_index *ix, const void *workspace, uint32_t B, uint64_t max_total_cands,
+                                        uint32_t k, uint64_t *total_cands, void *stream_)
+{
+    if (!ix || !workspace) return fail(FANN_EINVAL, "fann_search_lists_status: NULL argument");
+    if (!ix->codes || B == 0 || k == 0 || k > FANN_MAX_K) return fail(FANN_EINVAL, "fann_search_lists_status: bad argument");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    ListsHeader h;
+    CUDA_TRY(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    if (total_cands) *total_cands = h.total;
+    if (h.overflow)
+        return fail(FANN_EWORKSPACE, "the probed lists hold %llu candidate IDs, the workspace was sized for %llu (max_total_cands)",
+                    h.total, h.capacity);
+    ListsLayout l;
+    lists_layout(ix, B, max_total_cands, k, &l);
+    return fann_workspace_status(ix, (const char *)workspace + l.ws, stream);
+}
+
+struct ListsHostScratch { size_t queries, probes, lut, out_ids, out_dists, out_counts, ws, ws_bytes, total; };
+
+static void lists_host_layout(const fann_index *ix, uint32_t B, uint32_t dsub, uint32_t nprobe, uint64_t cap, uint32_t k,
+                              ListsHostScratch *h)
+{
+    ListsLayout l;
+    lists_layout(ix, B, cap, k, &l);
+    size_t o = 0;
+    h->queries = o;    o = align_up(o + (size_t)B * ix->M * dsub * 4, 256);
+    h->probes = o;     o = align_up(o + (size_t)B * nprobe * 4, 256);
+    h->lut = o;        o = align_up(o + (size_t)B * ix->M * 1024, 256);
+    h->out_ids = o;    o = align_up(o + (size_t)B * k * 4, 256);
+    h->out_dists = o;  o = align_up(o + (size_t)B * k * 4, 256);
+    h->out_counts = o; o = align_up(o + (size_t)B * 4, 256);
+    h->ws = o;         h->ws_bytes = l.total; o += l.total;
+    h->total = o;
+}
+
+extern "C" size_t fann_search_lists_host_scratch_bytes(const fann_index *ix, uint32_t B, uint32_t dsub, uint32_t nprobe,
+                                                       uint64_t max_total_cands, uint32_t k)
+{
+    if (!ix || !ix->codes || B == 0 || dsub == 0 || nprobe == 0 || k == 0 || k > FANN_MAX_K) {
+        fail(FANN_EINVAL, "fann_search_lists_host_scratch_bytes: bad argument");
+        return 0;
+    }
+    ListsHostScratch h;
+    lists_host_layout(ix, B, dsub, nprobe, max_total_cands, k, &h);
+    return h.total;
+}
+
+extern "C" int fann_search_lists_host(fann_index *ix, const float *queries_h, uint32_t B, const float *codebooks_d,
+                                      uint32_t dsub, const uint32_t *probes_h, uint32_t nprobe, uint64_t max_total_cands,
+                                      uint32_t k, uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h,
+                                      void *device_scratch, size_t scratch_bytes, void *stream_)
+{
+    if (!ix || !queries_h || !codebooks_d || !probes_h || !out_ids_h || !out_dists_h)
+        return fail(FANN_EINVAL, "fann_search_lists_host: NULL argument");
+    if (!ix->codes || !ix->list_offsets) return fail(FANN_EINVAL, "fann_search_lists_host: load codes and posting lists first");
+    if (B == 0 || dsub == 0 || nprobe == 0) return fail(FANN_EINVAL, "fann_search_lists_host: B, dsub or nprobe is 0");
+    if (k == 0 || k > FANN_MAX_K) return fail(FANN_EUNSUPPORTED, "fann_search_lists_host: k=%u", k);
+    ListsHostScratch h;
+    lists_host_layout(ix, B, dsub, nprobe, max_total_cands, k, &h);
+    if (!device_scratch || ((uintptr_t)device_scratch & 255) != 0 || scratch_bytes < h.total)
+        return fail(FANN_EWORKSPACE, "fann_search_lists_host: scratch has %zu bytes, %zu needed (256-byte aligned)",
+                    scratch_bytes, h.total);
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    char *s = (char *)device_scratch;
+    // PAPER.md:L125 step (4) with the metadata on the GPU: only the query vectors and nprobe list indices per query go up
+    CUDA_TRY(cudaMemcpyAsync(s + h.queries, queries_h, (size_t)B * ix->M * dsub * 4, cudaMemcpyHostToDevice, stream));
+    CUDA_TRY(cudaMemcpyAsync(s + h.probes, probes_h, (size_t)B * nprobe * 4, cudaMemcpyHostToDevice, stream));
+    int rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
+    if (rc != FANN_OK) return rc;
+    rc = fann_search_lists(ix, (const float *)(s + h.lut), B, (const uint32_t *)(s + h.probes), nprobe, max_total_cands, k,
+                           (uint32_t *)(s + h.out_ids), (float *)(s + h.out_dists), (uint32_t *)(s + h.out_counts), nullptr,
+                           s + h.ws, h.ws_bytes, stream);
+    if (rc != FANN_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+    if (out_counts_h)
+        CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
+    return fann_search_lists_status(ix, s + h.ws, B, max_total_cands, k, nullptr, stream);   // synchronises
+}
+
+// ---------------------------------------------------------------- NEXT-1: heuristic re-ranking
+
+extern "C" int fann_load_vectors(fann_index *ix, const void *vectors, uint64_t first, uint64_t n, uint64_t N_total,
+                                 uint32_t d, int elem_type, int src_is_device, void *stream_)
+{
+    if (!ix || !vectors) return fail(FANN_EINVAL, "fann_load_vectors: NULL argument");
+    if (d == 0 || N_total == 0) return fail(FANN_EINVAL, "fann_load_vectors: d and N_total must be > 0");
+    if (d > kRerankMaxDim) return fail(FANN_EUNSUPPORTED, "fann_load_vectors: d=%u > %u", d, kRerankMaxDim);
+    if (elem_type != FANN_ELEM_F32 && elem_type != FANN_ELEM_U8 && elem_type != FANN_ELEM_I8)
+        return fail(FANN_EUNSUPPORTED, "fann_load_vectors: elem_type %d", elem_type);
+    if (N_total >= 0xFFFFFFFFull) return fail(FANN_EUNSUPPORTED, "fann_load_vectors: N_total must be < 2^32-1");
+    if (first > N_total || n > N_total - first) return fail(FANN_EINVAL, "fann_load_vectors: rows outside N_total");
+    const size_t es = elem_type == FANN_ELEM_F32 ? 4 : 1;
+    if (((uintptr_t)vectors & (es - 1)) != 0) return fail(FANN_EINVAL, "fann_load_vectors: misaligned source");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (!ix->vectors) {
+        cudaError_t e = cudaMalloc(&ix->vectors, (size_t)N_total * d * es);
+        if (e != cudaSuccess) { ix->vectors = nullptr; return fail(FANN_ENOMEM, "fann_load_vectors: cudaMalloc: %s", cudaGetErrorString(e)); }
+        ix->vec_N = N_total; ix->vec_d = d; ix->vec_elem = elem_type;
+    } else if (N_total != ix->vec_N || d != ix->vec_d || elem_type != ix->vec_elem) {
+        return fail(FANN_EINVAL, "fann_load_vectors: (N_total, d, elem_type) differ from the first call");
+    }
+    if (n == 0) return FANN_OK;
+    CUDA_TRY(cudaMemcpyAsync((char *)ix->vectors + (size_t)first * d * es, vectors, (size_t)n * d * es,
+                             src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+    if (!src_is_device) CUDA_TRY(cudaStreamSynchronize(stream));
+    return FANN_OK;
+}
+
+extern "C" int fann_rerank(fann_index *ix, const float *queries, uint32_t B, const uint32_t *task_ids, uint32_t n,
+                           uint32_t batch_size, uint32_t k, float eps, uint32_t beta, uint32_t *out_ids, float *out_dists,
+                           uint32_t *out_counts, uint32_t *out_batches, uint32_t *out_reads, void *stream_)
+{
+    if (!ix || !queries || !task_ids || !out_ids || !out_dists || !out_counts)
+        return fail(FANN_EINVAL, "fann_rerank: NULL argument");
+    if (!ix->vectors) return fail(FANN_EINVAL, "fann_rerank: load the raw vectors first (fann_load_vectors)");
+    if (B == 0 || n == 0 || batch_size == 0 || k == 0 || beta == 0)
+        return fail(FANN_EINVAL, "fann_rerank: B, n, batch_size, k and beta must be > 0");
+    if (k > kRerankMaxK || n > kRerankMaxTasks)
+        return fail(FANN_EUNSUPPORTED, "fann_rerank: k=%u (max %u), n=%u (max %u)", k, kRerankMaxK, n, kRerankMaxTasks);
+    if (!(eps >= 0.f)) return fail(FANN_EINVAL, "fann_rerank: eps must be >= 0");
+    if ((((uintptr_t)queries | (uintptr_t)task_ids | (uintptr_t)out_ids | (uintptr_t)out_dists | (uintptr_t)out_counts |
+          (uintptr_t)out_batches | (uintptr_t)out_reads) & 3) != 0)
+        return fail(FANN_EINVAL, "fann_rerank: arrays must be 4-byte aligned");
+    if (batch_size > kRerankMaxBatch) batch_size = kRerankMaxBatch > n ? n : kRerankMaxBatch;
+    if (batch_size > n) batch_size = n;                         // one mini-batch holds every task
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    RerankParams p;
+    p.vectors = ix->vectors; p.N = ix->vec_N; p.d = ix->vec_d; p.queries = queries; p.tasks = task_ids;
+    p.n = n; p.batch_size = batch_size; p.k = k; p.beta = beta; p.eps = eps;
+    p.out_ids = out_ids; p.out_dists = out_dists; p.out_counts = out_counts; p.out_batches = out_batches; p.out_reads = out_reads;
+    const size_t smem = (size_t)((p.d + 3u) & ~3u) * 4 + (size_t)((n + 3u) & ~3u) * 4 + ((size_t)2 * k + batch_size) * 8;
+    switch (ix->vec_elem) {
+    case FANN_ELEM_F32: rerank_kernel<kElemF32><<<B, kRerankThreads, smem, stream>>>(p); break;
+    case FANN_ELEM_U8:  rerank_kernel<kElemU8><<<B, kRerankThreads, smem, stream>>>(p); break;
+    default:            rerank_kernel<kElemI8><<<B, kRerankThreads, smem, stream>>>(p); break;
+    }
+    ix->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return FANN_OK;
+}
+
+// ---------------------------------------------------------------- NEXT-4: page-level I/O dedup
+
+extern "C" int fann_load_page_table(fann_index *ix, const uint32_t *page_of, uint64_t N, uint64_t n_pages,
+                                    int src_is_device, void *stream_)
+{
+    if (!ix || !page_of) return fail(FANN_EINVAL, "fann_load_page_table: NULL argument");
+    if (N == 0 || N >= 0xFFFFFFFFull || n_pages == 0 || n_pages >= 0xFFFFFFFFull)
+        return fail(FANN_EINVAL, "fann_load_page_table: N and n_pages must be in 1 .. 2^32-2");
+    if (((uintptr_t)page_of & 3) != 0) return fail(FANN_EINVAL, "fann_load_page_table: page_of must be 4-byte aligned");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (ix->page_of) { cudaFree(ix->page_of); ix->page_of = nullptr; ix->page_N = 0; }
+    cudaError_t e = cudaMalloc(&ix->page_of, N * 4);
+    if (e != cudaSuccess) { ix->page_of = nullptr; return fail(FANN_ENOMEM, "fann_load_page_table: cudaMalloc: %s", cudaGetErrorString(e)); }
+    CUDA_TRY(cudaMemcpyAsync(ix->page_of, page_of, N * 4, src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+    if (!src_is_device) CUDA_TRY(cudaStreamSynchronize(stream));
+    ix->page_N = N; ix->n_pages = n_pages;
+    return FANN_OK;
+}
+
+extern "C" int fann_page_reads(fann_index *ix, const uint32_t *task_ids, uint32_t B, uint32_t n, uint32_t batch_size,
+                               const uint32_t *batches_run, const uint32_t *resident_bits, uint32_t *out_pages,
+                               uint32_t *out_batch_reads, uint32_t *out_total, void *stream_)
+{
+    if (!ix || !task_ids || !out_pages || !out_batch_reads || !out_total)
+        return fail(FANN_EINVAL, "fann_page_reads: NULL argument");
+    if (!ix->page_of) return fail(FANN_EINVAL, "fann_page_reads: load the vector -> page table first (fann_load_page_table)");
+    if (B == 0 || n == 0 || batch_size == 0) return fail(FANN_EINVAL, "fann_page_reads: B, n and batch_size must be > 0");
+    if (n > kPageMaxTasks) return fail(FANN_EUNSUPPORTED, "fann_page_reads: n=%u > %u", n, kPageMaxTasks);
+    if ((((uintptr_t)task_ids | (uintptr_t)batches_run | (uintptr_t)resident_bits | (uintptr_t)out_pages |
+          (uintptr_t)out_batch_reads | (uintptr_t)out_total) & 3) != 0)
+        return fail(FANN_EINVAL, "fann_page_reads: arrays must be 4-byte aligned");
+    if (batch_size > n) batch_size = n;
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    PageParams p;
+    p.page_of = ix->page_of; p.N = ix->page_N; p.n_pages = ix->n_pages; p.tasks = task_ids; p.n = n;
+    p.batch_size = batch_size; p.n_batches = (n + batch_size - 1) / batch_size; p.batches_run = batches_run;
+    p.resident = resident_bits; p.out_pages = out_pages; p.out_batch_reads = out_batch_reads; p.out_total = out_total;
+    uint32_t slots = 64;
+    while (slots < 2 * n) slots <<= 1;
+    page_reads_kernel<<<B, kPageThreads, (size_t)slots * 4, stream>>>(p, slots);
+    ix->launches++;
+    CUDA_TRY(cudaGetLastError());
+    return FANN_OK;
 }
 
 // ---------------------------------------------------------------- measurement

@@ -426,10 +426,46 @@ class Workload:
     cand_offsets: torch.Tensor             # [B+1] int64
     cand_ids: torch.Tensor                 # [total] int32 holding uint32 bit patterns
     stats: Dict[str, float] = field(default_factory=dict)
+    list_offsets: Optional[torch.Tensor] = None   # [n_lists + 1] int64  (keep_lists=True)
+    list_ids: Optional[torch.Tensor] = None       # [entries] int32
+    probes: Optional[torch.Tensor] = None         # [B, nprobe] int32: the lists each query probes, in probe order
+
+
+def make_raw_vectors(cfg: WorkloadConfig, seed: int, device="cpu", dtype=None) -> torch.Tensor:
+    """The N raw vectors the codes were encoded from ('data' stream; only meaningful for codes_mode == 'encode',
+    where code i is the nearest-centroid code of vector i), as fp32 or -- for integer-valued data -- uint8 / int8."""
+    kdata = stream_key(seed, cfg.name, "data")
+    want = dtype or {"u8": torch.uint8, "i8": torch.int8}.get(cfg.values, torch.float32)
+    out = torch.empty((cfg.N, cfg.d), dtype=want, device=device)
+    step = 1 << 16
+    for a in range(0, cfg.N, step):
+        n = min(step, cfg.N - a)
+        out[a:a + n] = draw_vectors(cfg, kdata, a, n, device).to(want)
+    return out
+
+
+def make_page_table(cfg: WorkloadConfig, seed: int, device="cpu", page_bytes: int = 4096, elem_bytes: int = 1):
+    """Vector -> SSD page in the *shape* of the paper's optimised layout: the raw vectors of a
+    posting list's home members are stored together, page after page, so vectors of one cluster share pages.
+    Distinct vector t (ordered by home list) sits in page t // per_page; IDs no list references follow.
+    Returns (page_of int32 [N], n_pages)."""
+    per_page = max(1, page_bytes // (cfg.d * elem_bytes))
+    home_sz = list_home_sizes(cfg, seed, device)
+    T = int(home_sz.sum())
+    page_of = torch.full((cfg.N,), -1, dtype=torch.int32, device=device)
+    step = 1 << 24
+    for a in range(0, T, step):
+        t = torch.arange(a, min(T, a + step), dtype=torch.int64, device=device)
+        page_of[vector_ids(cfg, seed, t)] = (t // per_page).to(torch.int32)
+    rest = torch.nonzero(page_of < 0, as_tuple=False).squeeze(1)
+    first_free = (T + per_page - 1) // per_page
+    page_of[rest] = (first_free + torch.arange(rest.numel(), dtype=torch.int64, device=device) // per_page).to(torch.int32)
+    n_pages = first_free + (rest.numel() + per_page - 1) // per_page
+    return page_of, int(n_pages)
 
 
 def make_workload(cfg: WorkloadConfig, seed: int = DEFAULT_SEED, device="cpu",
-                  with_codes: bool = True) -> Workload:
+                  with_codes: bool = True, keep_lists: bool = False) -> Workload:
     codebooks = make_codebooks(cfg, seed, device)
     queries = make_queries(cfg, seed, device)
     lists = make_lists(cfg, seed, device)
@@ -446,6 +482,7 @@ def make_workload(cfg: WorkloadConfig, seed: int = DEFAULT_SEED, device="cpu",
         "C_total": int(cand_offsets[-1]),
         "C_mean": float(per_q.mean()), "C_min": float(per_q.min()), "C_max": float(per_q.max()),
     }
+    kept = (lists.offsets, lists.ids, probes.to(torch.int32)) if keep_lists else (None, None, None)
     del lists
     codes = make_codes(cfg, seed, codebooks, device) if with_codes else None
-    return Workload(cfg, seed, queries, codebooks, codes, cand_offsets, cand_ids, stats)
+    return Workload(cfg, seed, queries, codebooks, codes, cand_offsets, cand_ids, stats, *kept)
