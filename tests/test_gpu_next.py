@@ -83,8 +83,14 @@ def test_search_lists_equals_oracle_and_the_id_path(fann, wl_int, wl_tiny):
         lut = ix.build_lut(w.queries.to(DEV), w.codebooks.to(DEV))
         o = ix.dedup_scan_topk(lut, w.cand_offsets.to(DEV), w.cand_ids.to(DEV), w.cfg.k, check=True)
         torch.cuda.synchronize()
-        assert np.array_equal(np_u32(o[0]), res[0]) and np.array_equal(o[1].cpu().numpy(), res[1])
         assert np.array_equal(np_u32(o[3]), res[3])
+        if w.cfg.integer_exact:
+            assert np.array_equal(np_u32(o[0]), res[0]) and np.array_equal(o[1].cpu().numpy(), res[1])
+        else:
+            # fp32 data: a row's summation order depends on the lane that scores it, and the order of the distinct
+            # list on which store wins a slot, so two runs agree within the band, not byte for byte
+            assert np.array_equal(np_u32(o[0]), res[0])
+            assert np.allclose(o[1].cpu().numpy(), res[1], rtol=2e-6, atol=0)
         ix.close()
 
 
