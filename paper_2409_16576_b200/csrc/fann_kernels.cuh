@@ -445,76 +445,103 @@ __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, ui
     return r;
 }
 
-constexpr int kDedupIdsPerThread = 8;                // IDs a thread holds per batch (two 16-byte loads)
-__host__ __device__ constexpr uint32_t dedup_table_off(uint32_t threads) { return 256 + 2 * threads * 4; }   // bookkeeping + two retry queues precede the table
+constexpr int kDedupIdsPerThread = 8;                // fresh IDs a thread holds per batch (two 16-byte loads)
+// bookkeeping (256 bytes, of which bytes 64..79 are a bucket that stays empty) + two retry queues of `threads`
+// (id, bucket address) pairs precede the table
+__host__ __device__ constexpr uint32_t dedup_table_off(uint32_t threads) { return 256 + 2 * threads * 8; }
 
 // PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel takes
 // a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-memory
-// pipe on this part (64x a plain load).  This kernel uses neither: open addressing with linear probing
-// in shared memory, advanced in CTA-wide rounds with no store in flight while anyone reads:
-//   probe  (reads only)  every pending ID walks its probe sequence to its own value (a repeat: done)
-//                        or to the first empty slot;
-//   write                every still-pending ID stores itself into the empty slot it found;
-//   verify (reads only)  one of several stores to a slot survived; the losers (a few per batch) enter a
-//                        small queue and are taken up again, one per thread, with the next batch.
-// A slot seen non-empty keeps its value for good, all copies of an ID walk the same sequence, so exactly
-// one slot ends up holding it.  Each CTA pass handles the IDs of one query that fall into one partition
-// (an ID range in ordered mode, a hash class in hashed mode), 8 per thread per batch, then compacts its
-// table in slot order into the query's distinct list.
+// pipe on this part (64x a plain load).  This kernel uses neither.  The table is an array of 16-byte
+// buckets of 4 slots; an ID's bucket is an order-preserving (or hashed) function of the ID, so one
+// 16-byte shared load shows every slot the ID can be in, and the CTA advances in rounds with no store in
+// flight while anyone reads:
+//   read   one load per ID: found in its bucket (a repeat: done), else the empty slot it will take (its
+//          home slot id & 3 if that is empty, else the first empty one), else -- bucket full -- the ID
+//          moves on to the next bucket through the retry queue;
+//   write  every ID that found an empty slot stores itself there;
+//   verify of several stores to one slot one survived; the losers (about 5 %) go to the retry queue.
+// The code is straight-line: nothing walks a probe sequence in a divergent loop.  A queued (ID, bucket)
+// pair is taken up again, one per thread, with the next batch.  A bucket seen full stays full, a slot seen
+// non-empty keeps its value, and all copies of an ID make the same choices from the same view, so exactly one
+// slot ends up holding it.  Each CTA pass handles the IDs of one query that fall into one partition (an ID
+// range in ordered mode, a hash class in hashed mode), 8 per thread per batch, then compacts its table in
+// bucket order into the query's distinct list.
 // T threads per CTA: 1024 (one CTA per SM, the whole shared memory as one table) or 512 (two CTAs per SM with half
 // the table each: one computes while the other waits at a barrier).
 template <int T>
 __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
 {
-    constexpr int R = kDedupIdsPerThread;
+    constexpr int R = kDedupIdsPerThread, NE = R + 1;          // entries per thread and batch: R fresh + 1 from the queue
+    constexpr uint32_t kNoSlot = 16;                           // "no empty slot in this bucket" as a byte offset
     extern __shared__ __align__(16) unsigned char smem[];
-    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);      // [0] item [1] out base [2,3] queue lengths [4] kEmpty [32..63] warp counts
+    // [0] out base [2,3] queue lengths [5] queue overflow [8..15], [24..31] the item of this pass and the next one:
+    // item, lo, span, bmul, nb  [16..19] a bucket that stays empty  [32..63] warp counts
+    uint32_t *misc = reinterpret_cast<uint32_t *>(smem);
     uint32_t *wsum = misc + 32, *qcnt = misc + 2;
-    uint32_t *queue = reinterpret_cast<uint32_t *>(smem + 256);              // two retry queues of T IDs
+    uint2 *queue = reinterpret_cast<uint2 *>(smem + 256);                    // two retry queues of T (id, bucket address)
     uint32_t *table = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T));
     const uint32_t tbl = (uint32_t)__cvta_generic_to_shared(table);
-    const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 4);   // a word that always holds kEmpty
+    const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 16);   // a bucket that always holds 4 x kEmpty
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t first = p.item_start[p.q_begin], last = p.item_start[p.q_end];
-    if (tid == 0) misc[4] = kEmpty;
+
+    // Thread 0 takes the next (query, partition) item off the work counter and does its 64-bit divisions (table
+    // geometry) for everybody, one pass ahead, so that nobody waits for this chain of dependent loads.
+    auto fetch_item = [&](uint32_t *slot) {
+        const uint32_t item = first + atomicAdd(p.counter, 1u);
+        slot[0] = item;
+        if (item >= last) return;
+        const uint2 it = p.items[item];
+        const uint32_t b = it.x, part = it.y, S = p.S[b];
+        const long long Cll = p.cand_offsets[b + 1] - p.cand_offsets[b];
+        const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;       // plan guarantees C / S <= 0.75 nslots_max
+        const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
+        // table sized to the partition, never more than the CTA can hold: 2 slots per expected candidate; 1.5
+        // where the count is exact (about 0.4 full after dedup)
+        uint32_t nslots = p.nslots_max;
+        const unsigned long long want = ((pre ? (unsigned long long)p.bucket_cnt[item] * 3 / 2
+                                              : (unsigned long long)(C / S + 1) * 2) + 128) & ~3ull;
+        if (want < nslots) nslots = (uint32_t)want;
+        const uint32_t nb = nslots >> 2;                       // buckets
+        // ordered mode: this partition owns the IDs of class `part`, a range [lo, lo + span);
+        // bucket = (id - lo) * nb / span
+        uint32_t lo = 0, span = 0, bmul = 0;
+        if (p.mode[b] != kModeHashed) {
+            const uint32_t class_mul = ordered_class_mul(p.N, S);
+            lo = ordered_class_start(class_mul, part, p.N);
+            span = ordered_class_start(class_mul, part + 1, p.N) - lo;
+            // span <= nb (tiny N): bucket = id - lo - 1 or 0, still order-preserving and inside the table
+            bmul = span > nb ? (uint32_t)(((unsigned long long)nb << 32) / span) : 0xFFFFFFFFu;
+        }
+        slot[1] = lo; slot[2] = span; slot[3] = bmul; slot[4] = nb;
+    };
+    if (tid < 4) misc[16 + tid] = kEmpty;
+    if (tid == 0) { misc[5] = 0; fetch_item(misc + 8); }
+    uint32_t sel = 0;
 
     for (;;) {
-        __syncthreads();                                       // previous item fully done
-        if (tid == 0) misc[0] = first + atomicAdd(p.counter, 1u);
-        __syncthreads();
-        const uint32_t item = misc[0];
+        __syncthreads();                                       // previous item fully done; this one's geometry is there
+        const uint32_t *cur_item = misc + (sel ? 24 : 8);
+        const uint32_t item = cur_item[0];
         if (item >= last) break;
+        const uint32_t lo = cur_item[1], span = cur_item[2], bmul = cur_item[3], nb = cur_item[4];
+        if (tid == 0) fetch_item(misc + (sel ? 8 : 24));
+        sel ^= 1u;
         const uint2 it = p.items[item];
         const uint32_t b = it.x, part = it.y, S = p.S[b];
         const bool hashed = p.mode[b] == kModeHashed;
         const long long off0 = p.cand_offsets[b];
         const long long Cll = p.cand_offsets[b + 1] - off0;
-        const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;       // plan guarantees C / S <= 0.75 nslots_max
-
+        const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;
         // pre-partitioned: this item's IDs were split off by partition_kernel; every ID read is ours
         const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
         const uint32_t Cin = pre ? p.bucket_cnt[item] : C;     // IDs this pass reads
-
-        // table sized to the partition, never more than the CTA can hold
-        uint32_t nslots = p.nslots_max;
-        {
-            // 2 slots per expected candidate; 1.5 where the count is exact (about 0.4 full after dedup)
-            const unsigned long long want = ((pre ? (unsigned long long)Cin * 3 / 2 : (unsigned long long)(C / S + 1) * 2) + 128) & ~3ull;
-            if (want < nslots) nslots = (uint32_t)want;
-        }
-        // ordered mode: this partition owns the IDs of class `part`, a range [lo, lo + span);
-        // slot = (id - lo) * nslots / span
-        uint32_t lo = 0, span = 0, slot_mul = 0, class_mul = 0;
-        if (!hashed) {
-            class_mul = ordered_class_mul(p.N, S);
-            lo = ordered_class_start(class_mul, part, p.N);
-            span = ordered_class_start(class_mul, part + 1, p.N) - lo;
-            slot_mul = span > nslots ? (uint32_t)(((unsigned long long)nslots << 32) / span) : 0u;   // 0: slot = id - lo
-        }
         {
             uint4 *t4 = reinterpret_cast<uint4 *>(table);
             const uint4 e4 = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
-            for (uint32_t i = tid; i < (nslots >> 2); i += T) t4[i] = e4;
+            for (uint32_t i = tid; i < nb; i += T) t4[i] = e4;
         }
 
         // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list.
@@ -530,130 +557,169 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
             if (v < nvec) return load_ids4(ids, 4ll * v - shift, Cin);
             return none4;
         };
-        // shared-memory byte address of the home slot of a valid ID of this partition
-        auto place = [&](uint32_t x) -> uint32_t {
-            if (!hashed) return tbl + ((slot_mul ? __umulhi(x - lo, slot_mul) : x - lo) << 2);
+        // hashed mode: bucket and home slot of a valid ID
+        auto hash_of = [&](uint32_t x) -> uint32_t {
             uint32_t a = hash_round1(x);
             a = (a ^ (a >> 15)) * 0x846ca68bU;
-            a ^= a >> 16;
-            return tbl + (__umulhi(a, nslots) << 2);
+            return a ^ (a >> 16);
         };
-        const uint32_t tbl_end = tbl + (nslots << 2);
+        // byte offset of the slot an ID tries first inside its bucket: low bits the bucket index does not use
+        auto home_of = [&](uint32_t x) -> uint32_t { return ((hashed ? hash_of(x) : x - lo) << 2) & 12u; };
+        // the bucket an ID of this partition looks at first
+        auto bucket_of = [&](uint32_t x) -> uint32_t { return tbl + ((hashed ? __umulhi(hash_of(x), nb) : __umulhi(x - lo, bmul)) << 4); };
+        const uint32_t tbl_end = tbl + (nb << 4);
+        auto next_bucket = [&](uint32_t a) -> uint32_t { return a + 16 == tbl_end ? tbl : a + 16; };
+        // One look at bucket `a` for ID `x` (kIdNone looks at the empty bucket and "finds itself" there):
+        // x is there (a repeat): x becomes kIdNone; else returns the slot x will store itself to (its home slot if
+        // that is empty, else the first empty one), or none_addr with x unchanged if the bucket is full of other
+        // IDs.  `home` = byte offset of the slot tried first.
+        auto look = [&](uint32_t &x, uint32_t a, uint32_t home) -> uint32_t {
+            const uint4 v = lds_u128(a);
+            const uint32_t hv = lds_u32(a + home);
+            const bool found = v.x == x || v.y == x || v.z == x || v.w == x;
+            uint32_t off = kNoSlot;
+            off = v.w == kEmpty ? 12u : off;
+            off = v.z == kEmpty ? 8u : off;
+            off = v.y == kEmpty ? 4u : off;
+            off = v.x == kEmpty ? 0u : off;
+            off = hv == kEmpty ? home : off;
+            if (found) x = kIdNone;
+            return (found || off == kNoSlot) ? none_addr : a + off;
+        };
+        // Places the entries of this thread whose bit is set in `keep` (t[j] = bucket to start at), each walking
+        // its bucket sequence in the same three phases, until every thread of the CTA is done.  Used for what the
+        // queue holds when the list is exhausted (NK = 1, one entry per thread), and for entries that found the
+        // queue full (IDs chosen to collide).
+        auto place_kept = [&](auto &id, auto &t, uint32_t keep) {
+            constexpr int NK = sizeof(id) / sizeof(id[0]);
+            for (;;) {
+#pragma unroll
+                for (int j = 0; j < NK; ++j) {
+                    if (!(keep >> j & 1u)) continue;
+                    const uint32_t home = home_of(id[j]);
+                    uint32_t a = t[j] & ~15u, steps = 0;
+                    for (;;) {
+                        const uint32_t r = look(id[j], a, home);
+                        if (id[j] == kIdNone) { keep &= ~(1u << j); break; }
+                        if (r != none_addr) { a = r; break; }
+                        a = next_bucket(a);
+                        if (++steps > nb) {                    // the table is full of other IDs: give up on this one
+                            atomicOr(&p.hdr->status, kStatusTableFull);
+                            keep &= ~(1u << j);
+                            break;
+                        }
+                    }
+                    t[j] = a;
+                }
+                if (!__syncthreads_or(keep != 0)) break;       // all reads done
+#pragma unroll
+                for (int j = 0; j < NK; ++j)
+                    if (keep >> j & 1u) sts_u32(t[j], id[j]);
+                __syncthreads();                               // all stores done
+#pragma unroll
+                for (int j = 0; j < NK; ++j)
+                    if ((keep >> j & 1u) && lds_u32(t[j]) == id[j]) keep &= ~(1u << j);
+            }
+        };
         uint4 nxt0 = load_vec(tid), nxt1 = load_vec(tid + T);   // this thread's vectors of the next batch
         if (tid == 0) { qcnt[0] = 0; qcnt[1] = 0; }
         __syncthreads();                                       // table cleared, queues empty
 
-        // Batches of 8 fresh IDs per thread plus one ID from the retry queue (IDs that lost a store race
-        // in the batch before).  After the list is exhausted the loop runs on until the queue is empty.
-        // sa[j] is the shared-memory byte address of the slot ID j looks at.  An absent ID (kIdNone) looks
-        // at `none_addr`, a word that always holds kEmpty == kIdNone: it "finds itself" there, so probe and
-        // verify need no special case and no predicated loads.
         uint32_t qin = 0, qn = 0;                              // queue read by this batch, its length
-        for (uint32_t vbase = 0; vbase < nvec || qn; vbase += 2 * T) {
-            uint32_t id[R + 1] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w, kIdNone};
-            uint32_t sa[R + 1];
+        for (uint32_t vbase = 0; vbase < nvec; vbase += 2 * T) {
+            uint32_t id[NE] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w, kIdNone};
+            uint32_t t[NE];                                    // slot to store to, none_addr = nothing to store
             nxt0 = load_vec(vbase + 2 * T + tid);
             nxt1 = load_vec(vbase + 3 * T + tid);
-            if (!hashed) {
+            uint2 *qpush = queue + (qin ^ 1u) * T;
+            uint32_t *qpush_cnt = qcnt + (qin ^ 1u);
+            // ---- read: one look per entry
 #pragma unroll
-                for (int j = 0; j < R; ++j) {
+            for (int j = 0; j < R; ++j) {
+                uint32_t bk, home;
+                bool mine;
+                if (!hashed) {
                     const uint32_t x = id[j] - lo;
-                    const uint32_t a = tbl + ((slot_mul ? __umulhi(x, slot_mul) : x) << 2);
                     // class test: drops other classes, IDs >= N and kIdNone (lo + span <= N); a
                     // pre-partitioned bucket holds only this class, so there it drops just the padding
-                    const bool mine = x < span;
-                    sa[j] = mine ? a : none_addr;
-                    if (!mine) id[j] = kIdNone;
-                }
-            } else {
-#pragma unroll
-                for (int j = 0; j < R; ++j) {
+                    mine = x < span;
+                    bk = __umulhi(x, bmul);
+                    home = (x << 2) & 12u;
+                } else {
                     const uint32_t x = id[j];
-                    const bool mine = (uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part);
-                    sa[j] = mine ? place(x) : none_addr;
-                    if (!mine) id[j] = kIdNone;
+                    mine = (uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part);
+                    const uint32_t h = hash_of(x);
+                    bk = __umulhi(h, nb);                      // the high bits of h
+                    home = (h << 2) & 12u;                     // the low bits
+                }
+                if (!mine) id[j] = kIdNone;
+                t[j] = look(id[j], mine ? tbl + (bk << 4) : none_addr, home);
+            }
+            uint32_t aq = none_addr;                           // the bucket the queued entry looks at
+            {
+                uint32_t home = 0;
+                if (tid < qn) {
+                    const uint2 e = queue[qin * T + tid];
+                    id[R] = e.x; aq = e.y;
+                    home = home_of(e.x);
+                }
+                t[R] = look(id[R], aq, home);
+            }
+            uint32_t all = id[0];
+#pragma unroll
+            for (int j = 1; j < NE; ++j) all &= id[j];
+            const bool any_left = __syncthreads_or(all != kIdNone);   // all reads done
+            if (tid == 0) qcnt[qin] = 0;                       // drained queue: its length was read before this barrier
+            uint32_t keep = 0;                                 // entries that found the queue full
+            if (any_left) {
+                // ---- write
+#pragma unroll
+                for (int j = 0; j < NE; ++j)
+                    if (t[j] != none_addr) sts_u32(t[j], id[j]);
+                __syncthreads();                               // all stores done
+                // ---- verify: of several stores to one slot one survived.  Losers (same bucket again) and IDs
+                // whose bucket was full (next bucket) go to the queue the next batch reads; an entry that is done
+                // reads kEmpty == its id from the empty bucket.  A full queue (IDs chosen to collide) raises
+                // misc[5]; the ID then stays with its thread and is placed right after this batch.
+#pragma unroll
+                for (int j = 0; j < NE; ++j) {
+                    const uint32_t cur = lds_u32(t[j]);
+                    if (cur != id[j]) {
+                        if (t[j] == none_addr) t[j] = next_bucket(j < R ? bucket_of(id[j]) : aq);
+                        const uint32_t pos = atomicAdd(qpush_cnt, 1u);
+                        if (pos < (uint32_t)T) qpush[pos] = make_uint2(id[j], t[j] & ~15u);
+                        else { misc[5] = 1; keep |= 1u << j; }
+                    }
                 }
             }
-            sa[R] = none_addr;
-            if (tid < qn) { id[R] = queue[qin * T + tid]; sa[R] = place(id[R]); }
-            uint32_t *qpush = queue + (qin ^ 1u) * T;
-            for (;;) {
-                // probe (reads only): to the ID itself (a repeat) or to the first empty slot
-                uint32_t cur[R + 1];
-#pragma unroll
-                for (int j = 0; j <= R; ++j) cur[j] = lds_u32(sa[j]);
-                bool unres = false;
-#pragma unroll
-                for (int j = 0; j <= R; ++j) {
-                    unres |= cur[j] != id[j] && cur[j] != kEmpty;
-                    if (cur[j] == id[j]) id[j] = kIdNone;
-                }
-                if (unres) {                                   // some slot held another ID: walk on
-#pragma unroll
-                    for (int j = 0; j <= R; ++j) {
-                        if (cur[j] == kEmpty || id[j] == kIdNone) continue;
-                        uint32_t c, a = sa[j], steps = 0;
-                        do {
-                            a += 4;
-                            if (a == tbl_end) a = tbl;
-                            c = lds_u32(a);
-                            if (++steps > nslots) {            // table full of other IDs: give up on this one
-                                atomicOr(&p.hdr->status, kStatusTableFull);
-                                c = id[j];
-                            }
-                        } while (c != id[j] && c != kEmpty);
-                        sa[j] = a;
-                        if (c == id[j]) { id[j] = kIdNone; sa[j] = none_addr; }
-                    }
-                }
-                uint32_t all = id[0];
-#pragma unroll
-                for (int j = 1; j <= R; ++j) all &= id[j];
-                const bool any_store = __syncthreads_or(all != kIdNone);   // all reads done
-                if (tid == 0) qcnt[qin] = 0;                   // drained queue: its length was read before this barrier
-                if (!any_store) break;                         // nothing to store: batch done
-#pragma unroll
-                for (int j = 0; j <= R; ++j)
-                    if (id[j] != kIdNone) sts_u32(sa[j], id[j]);
-                __syncthreads();                               // all stores done
-                // verify (reads only): of several stores to one slot one survived
-#pragma unroll
-                for (int j = 0; j <= R; ++j) cur[j] = lds_u32(sa[j]);
-                all = kIdNone;
-#pragma unroll
-                for (int j = 0; j <= R; ++j) {
-                    if (cur[j] == id[j]) id[j] = kIdNone;
-                    all &= id[j];
-                }
-                if (all != kIdNone) {                          // losers: retry with the next batch
-#pragma unroll
-                    for (int j = 0; j <= R; ++j) {
-                        if (id[j] == kIdNone) continue;
-                        const uint32_t pos = atomicAdd(&qcnt[qin ^ 1u], 1u);
-                        if (pos < (uint32_t)T) { qpush[pos] = id[j]; id[j] = kIdNone; sa[j] = none_addr; }
-                    }
-                    all = id[0];
-#pragma unroll
-                    for (int j = 1; j <= R; ++j) all &= id[j];
-                }
-                if (!__syncthreads_or(all != kIdNone)) break;  // queue full (IDs chosen to collide): go round again
+            __syncthreads();                                   // queue complete; misc[5] final
+            if (misc[5]) {
+                place_kept(id, t, keep);
+                if (tid == 0) misc[5] = 0;
+                __syncthreads();
             }
             qin ^= 1u;                                         // the queue just filled is the next batch's input
             qn = qcnt[qin];
             if (qn > (uint32_t)T) qn = T;
         }
+        if (qn) {                                              // list exhausted: place what the queue still holds
+            uint32_t id[1] = {kIdNone}, t[1] = {none_addr};
+            if (tid < qn) {
+                const uint2 e = queue[qin * T + tid];
+                id[0] = e.x; t[0] = e.y;
+            }
+            place_kept(id, t, tid < qn ? 1u : 0u);
+        }
 
-        // compact the table in slot order: count per warp range, scan, write
+        // compact the table in bucket order: count per warp range, scan, write
         {
-            const uint4 *t4 = reinterpret_cast<const uint4 *>(table);
-            const uint32_t n4 = nslots >> 2;
-            const uint32_t chunk = ((n4 + T - 1) / T) * 32;   // vectors per warp, multiple of 32
-            const uint32_t v0 = warp * chunk < n4 ? warp * chunk : n4;
-            const uint32_t v1 = v0 + chunk < n4 ? v0 + chunk : n4;
+            const uint32_t chunk = ((nb + T - 1) / T) * 32;   // buckets per warp, multiple of 32
+            const uint32_t v0 = warp * chunk < nb ? warp * chunk : nb;
+            const uint32_t v1 = v0 + chunk < nb ? v0 + chunk : nb;
             uint32_t c = 0;
             for (uint32_t v = v0 + lane; v < v1; v += 32) {
-                const uint4 t = t4[v];
-                c += (t.x != kEmpty) + (t.y != kEmpty) + (t.z != kEmpty) + (t.w != kEmpty);
+                const uint4 w = lds_u128(tbl + (v << 4));
+                c += (w.x != kEmpty) + (w.y != kEmpty) + (w.z != kEmpty) + (w.w != kEmpty);
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
@@ -669,24 +735,24 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
                     if (lane >= o) incl += u;
                 }
                 wsum[lane] = incl - wv;                        // exclusive
-                if (lane == 31) misc[1] = incl ? atomicAdd(p.uniq_counts + b, incl) : 0u;
+                if (lane == 31) misc[0] = incl ? atomicAdd(p.uniq_counts + b, incl) : 0u;
             }
             __syncthreads();
-            // 128 slots per warp step, written word-plane by word-plane (slots 4l of all lanes, then 4l+1, ...):
-            // ascending between steps, a fixed shuffle inside one -- four ballots instead of a warp scan
-            uint32_t *out = p.uniq_ids + off0 + misc[1] + wsum[warp];
-            const uint32_t lt_mask = (1u << lane) - 1u;
+            // one bucket per lane and step: the lane's distinct IDs go out side by side at the warp's running
+            // position plus the count of the lanes below (three ballots on the bits of the lane's count, 0..4)
+            uint32_t *out = p.uniq_ids + off0 + misc[0] + wsum[warp];
             for (uint32_t vb = v0; vb < v1; vb += 32) {
                 const uint32_t v = vb + lane;
-                const uint4 t = v < v1 ? t4[v] : make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
-                const uint32_t b0 = __ballot_sync(0xffffffffu, t.x != kEmpty), b1 = __ballot_sync(0xffffffffu, t.y != kEmpty);
-                const uint32_t b2 = __ballot_sync(0xffffffffu, t.z != kEmpty), b3 = __ballot_sync(0xffffffffu, t.w != kEmpty);
-                const uint32_t c1 = __popc(b0), c2 = c1 + __popc(b1), c3 = c2 + __popc(b2);
-                if (t.x != kEmpty) out[__popc(b0 & lt_mask)] = t.x;
-                if (t.y != kEmpty) out[c1 + __popc(b1 & lt_mask)] = t.y;
-                if (t.z != kEmpty) out[c2 + __popc(b2 & lt_mask)] = t.z;
-                if (t.w != kEmpty) out[c3 + __popc(b3 & lt_mask)] = t.w;
-                out += c3 + __popc(b3);
+                const uint4 w = lds_u128(v < v1 ? tbl + (v << 4) : none_addr);
+                const uint32_t px = w.x != kEmpty, py = px + (w.y != kEmpty), pz = py + (w.z != kEmpty), n = pz + (w.w != kEmpty);
+                const uint32_t b0 = __ballot_sync(0xffffffffu, n & 1u), b1 = __ballot_sync(0xffffffffu, n & 2u);
+                const uint32_t b2 = __ballot_sync(0xffffffffu, n & 4u);
+                uint32_t *o = out + (__popc(b0 & lt_mask) + 2 * __popc(b1 & lt_mask) + 4 * __popc(b2 & lt_mask));
+                if (w.x != kEmpty) o[0] = w.x;
+                if (w.y != kEmpty) o[px] = w.y;
+                if (w.z != kEmpty) o[py] = w.z;
+                if (w.w != kEmpty) o[pz] = w.w;
+                out += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
             }
         }
     }
