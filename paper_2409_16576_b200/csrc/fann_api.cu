@@ -206,8 +206,8 @@ extern "C" int fann_create(fann_index **out, int device)
     if (scan_max > smem_optin)
         return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
                     smem_optin, scan_max);
-    CUDA_TRY(cudaFuncSetAttribute(dedup_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
-    CUDA_TRY(cudaFuncSetAttribute(dedup_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin));
+    CUDA_TRY((cudaFuncSetAttribute(dedup_kernel<1024, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)));
+    CUDA_TRY((cudaFuncSetAttribute(dedup_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)));
     const int ring_max = (int)scan_smem_bytes(4096, 3);
     if (ring_max > smem_optin)
         return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
@@ -514,8 +514,8 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
             CUDA_TRY(cudaGetLastError());
         }
         dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
-        if (g.dedup_threads == 512) dedup_kernel<512><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
-        else dedup_kernel<1024><<<ix->num_sms, 1024, g.dedup_smem, stream>>>(dp);
+        if (g.dedup_threads == 512) dedup_kernel<512, 8><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
+        else dedup_kernel<1024, 8><<<ix->num_sms, 1024, g.dedup_smem, stream>>>(dp);
         if (timing) cudaEventRecord(ix->ev_dedup[c][1], stream);
         ix->launches++;
         CUDA_TRY(cudaGetLastError());

@@ -61,6 +61,16 @@ __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
     asm volatile("st.shared.u32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
 }
 
+__device__ __forceinline__ void sts_u128(uint32_t addr, uint4 v)
+{
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" :: "r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ uint2 lds_u64(uint32_t addr)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
+    return v;
+}
 __device__ __forceinline__ uint4 lds_u128(uint32_t addr)
 {
     uint4 v;
@@ -448,7 +458,10 @@ __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, ui
 constexpr int kDedupIdsPerThread = 8;                // fresh IDs a thread holds per batch (two 16-byte loads)
 // bookkeeping (256 bytes, of which bytes 64..79 are a bucket that stays empty) + two retry queues of `threads`
 // (id, bucket address) pairs precede the table
-__host__ __device__ constexpr uint32_t dedup_table_off(uint32_t threads) { return 256 + 2 * threads * 8; }
+constexpr int kDedupBucketSlots = 4;                 // slots per bucket (2: one 8-byte look, 4: one 16-byte look)
+constexpr int kDedupQueuePer8 = kDedupBucketSlots == 2 ? 2 : 1;   // queued entries a thread takes up per batch, per 8 fresh IDs
+// `shape` = threads x fresh IDs per thread / 8: 1024 (one CTA per SM) or 512 (two CTAs per SM)
+__host__ __device__ constexpr uint32_t dedup_table_off(uint32_t shape) { return 256 + 2 * kDedupQueuePer8 * shape * 8; }
 
 // PAPER.md:L127 "it first deduplicates them", L210 "parallel hash algorithm".  The paper's kernel takes
 // a spinlock per hash entry; an atomicCAS per ID costs about 2 cycles per lane of the shared-memory
@@ -469,18 +482,21 @@ __host__ __device__ constexpr uint32_t dedup_table_off(uint32_t threads) { retur
 // bucket order into the query's distinct list.
 // T threads per CTA: 1024 (one CTA per SM, the whole shared memory as one table) or 512 (two CTAs per SM with half
 // the table each: one computes while the other waits at a barrier).
-template <int T>
-__global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
+template <int T, int R>
+__global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const DedupParams p)
 {
-    constexpr int R = kDedupIdsPerThread, NE = R + 1;          // entries per thread and batch: R fresh + 1 from the queue
-    constexpr uint32_t kNoSlot = 16;                           // "no empty slot in this bucket" as a byte offset
+    constexpr int BS = kDedupBucketSlots, BSH = BS == 2 ? 3 : 4;   // slots per bucket, log2 of its bytes
+    constexpr int NV = R / 4, NQ = kDedupQueuePer8 * R / 8, NE = R + NQ;   // per thread and batch: NV vectors = R fresh IDs + NQ from the queue
+    constexpr uint32_t QCAP = NQ * T;                          // entries one retry queue holds
+    constexpr uint32_t kNoSlot = 4 * BS;                       // "no empty slot in this bucket" as a byte offset
+    constexpr uint32_t kBucketMask = ~(4u * BS - 1u);
     extern __shared__ __align__(16) unsigned char smem[];
     // [0] out base [2,3] queue lengths [5] queue overflow [8..15], [24..31] the item of this pass and the next one:
     // item, lo, span, bmul, nb  [16..19] a bucket that stays empty  [32..63] warp counts
     uint32_t *misc = reinterpret_cast<uint32_t *>(smem);
     uint32_t *wsum = misc + 32, *qcnt = misc + 2;
-    uint2 *queue = reinterpret_cast<uint2 *>(smem + 256);                    // two retry queues of T (id, bucket address)
-    uint32_t *table = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T));
+    uint2 *queue = reinterpret_cast<uint2 *>(smem + 256);                    // two retry queues of QCAP (id, bucket address)
+    uint32_t *table = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T * R / 8));
     const uint32_t tbl = (uint32_t)__cvta_generic_to_shared(table);
     const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 16);   // a bucket that always holds 4 x kEmpty
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -504,7 +520,7 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
         const unsigned long long want = ((pre ? (unsigned long long)p.bucket_cnt[item] * 3 / 2
                                               : (unsigned long long)(C / S + 1) * 2) + 128) & ~3ull;
         if (want < nslots) nslots = (uint32_t)want;
-        const uint32_t nb = nslots >> 2;                       // buckets
+        const uint32_t nb = nslots / BS;                       // buckets
         // ordered mode: this partition owns the IDs of class `part`, a range [lo, lo + span);
         // bucket = (id - lo) * nb / span
         uint32_t lo = 0, span = 0, bmul = 0;
@@ -519,9 +535,14 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
     };
     if (tid < 4) misc[16 + tid] = kEmpty;
     if (tid == 0) { misc[5] = 0; fetch_item(misc + 8); }
+    {   // the table starts empty; every pass leaves it empty again (the compaction clears what it reads)
+        const uint4 e4 = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
+        for (uint32_t i = tid; i < (p.nslots_max >> 2); i += T) reinterpret_cast<uint4 *>(table)[i] = e4;
+    }
     uint32_t sel = 0;
 
     for (;;) {
+        if (tid == 0) { qcnt[0] = 0; qcnt[1] = 0; }            // nobody reads them between the last batch and here
         __syncthreads();                                       // previous item fully done; this one's geometry is there
         const uint32_t *cur_item = misc + (sel ? 24 : 8);
         const uint32_t item = cur_item[0];
@@ -538,11 +559,6 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
         // pre-partitioned: this item's IDs were split off by partition_kernel; every ID read is ours
         const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
         const uint32_t Cin = pre ? p.bucket_cnt[item] : C;     // IDs this pass reads
-        {
-            uint4 *t4 = reinterpret_cast<uint4 *>(table);
-            const uint4 e4 = make_uint4(kEmpty, kEmpty, kEmpty, kEmpty);
-            for (uint32_t i = tid; i < nb; i += T) t4[i] = e4;
-        }
 
         // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list.
         // Vectors [v_in0, v_in1) lie wholly inside the list and are read with one 16-byte load.
@@ -564,25 +580,34 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
             return a ^ (a >> 16);
         };
         // byte offset of the slot an ID tries first inside its bucket: low bits the bucket index does not use
-        auto home_of = [&](uint32_t x) -> uint32_t { return ((hashed ? hash_of(x) : x - lo) << 2) & 12u; };
+        auto home_of = [&](uint32_t x) -> uint32_t { return ((hashed ? hash_of(x) : x - lo) << 2) & (4u * BS - 4u); };
         // the bucket an ID of this partition looks at first
-        auto bucket_of = [&](uint32_t x) -> uint32_t { return tbl + ((hashed ? __umulhi(hash_of(x), nb) : __umulhi(x - lo, bmul)) << 4); };
-        const uint32_t tbl_end = tbl + (nb << 4);
-        auto next_bucket = [&](uint32_t a) -> uint32_t { return a + 16 == tbl_end ? tbl : a + 16; };
+        auto bucket_of = [&](uint32_t x) -> uint32_t { return tbl + ((hashed ? __umulhi(hash_of(x), nb) : __umulhi(x - lo, bmul)) << BSH); };
+        const uint32_t tbl_end = tbl + (nb << BSH);
+        auto next_bucket = [&](uint32_t a) -> uint32_t { return a + 4 * BS == tbl_end ? tbl : a + 4 * BS; };
         // One look at bucket `a` for ID `x` (kIdNone looks at the empty bucket and "finds itself" there):
         // x is there (a repeat): x becomes kIdNone; else returns the slot x will store itself to (its home slot if
         // that is empty, else the first empty one), or none_addr with x unchanged if the bucket is full of other
         // IDs.  `home` = byte offset of the slot tried first.
         auto look = [&](uint32_t &x, uint32_t a, uint32_t home) -> uint32_t {
-            const uint4 v = lds_u128(a);
-            const uint32_t hv = lds_u32(a + home);
-            const bool found = v.x == x || v.y == x || v.z == x || v.w == x;
+            bool found;
             uint32_t off = kNoSlot;
-            off = v.w == kEmpty ? 12u : off;
-            off = v.z == kEmpty ? 8u : off;
-            off = v.y == kEmpty ? 4u : off;
-            off = v.x == kEmpty ? 0u : off;
-            off = hv == kEmpty ? home : off;
+            if (BS == 4) {
+                const uint4 v = lds_u128(a);
+                const uint32_t hv = lds_u32(a + home);
+                found = v.x == x || v.y == x || v.z == x || v.w == x;
+                off = v.w == kEmpty ? 12u : off;
+                off = v.z == kEmpty ? 8u : off;
+                off = v.y == kEmpty ? 4u : off;
+                off = v.x == kEmpty ? 0u : off;
+                off = hv == kEmpty ? home : off;
+            } else {
+                const uint2 v = lds_u64(a);
+                found = v.x == x || v.y == x;
+                const uint32_t hv = home ? v.y : v.x, ov = home ? v.x : v.y;
+                off = ov == kEmpty ? home ^ 4u : off;
+                off = hv == kEmpty ? home : off;
+            }
             if (found) x = kIdNone;
             return (found || off == kNoSlot) ? none_addr : a + off;
         };
@@ -597,7 +622,7 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
                 for (int j = 0; j < NK; ++j) {
                     if (!(keep >> j & 1u)) continue;
                     const uint32_t home = home_of(id[j]);
-                    uint32_t a = t[j] & ~15u, steps = 0;
+                    uint32_t a = t[j] & kBucketMask, steps = 0;
                     for (;;) {
                         const uint32_t r = look(id[j], a, home);
                         if (id[j] == kIdNone) { keep &= ~(1u << j); break; }
@@ -621,49 +646,56 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
                     if ((keep >> j & 1u) && lds_u32(t[j]) == id[j]) keep &= ~(1u << j);
             }
         };
-        uint4 nxt0 = load_vec(tid), nxt1 = load_vec(tid + T);   // this thread's vectors of the next batch
-        if (tid == 0) { qcnt[0] = 0; qcnt[1] = 0; }
-        __syncthreads();                                       // table cleared, queues empty
+        uint4 nxt[NV];                                         // this thread's vectors of the next batch
+#pragma unroll
+        for (int i = 0; i < NV; ++i) nxt[i] = load_vec(tid + i * T);
+        // (no barrier here: the table is empty since the last pass's compaction, which the barrier at the top of
+        // the loop closed; the queue lengths are reset there too)
 
         uint32_t qin = 0, qn = 0;                              // queue read by this batch, its length
-        for (uint32_t vbase = 0; vbase < nvec; vbase += 2 * T) {
-            uint32_t id[NE] = {nxt0.x, nxt0.y, nxt0.z, nxt0.w, nxt1.x, nxt1.y, nxt1.z, nxt1.w, kIdNone};
-            uint32_t t[NE];                                    // slot to store to, none_addr = nothing to store
-            nxt0 = load_vec(vbase + 2 * T + tid);
-            nxt1 = load_vec(vbase + 3 * T + tid);
-            uint2 *qpush = queue + (qin ^ 1u) * T;
+        for (uint32_t vbase = 0; vbase < nvec; vbase += NV * T) {
+            uint32_t id[NE], t[NE];                            // t: slot to store to, none_addr = nothing to store
+#pragma unroll
+            for (int i = 0; i < NV; ++i) {
+                id[4 * i] = nxt[i].x; id[4 * i + 1] = nxt[i].y; id[4 * i + 2] = nxt[i].z; id[4 * i + 3] = nxt[i].w;
+                nxt[i] = load_vec(vbase + (NV + i) * T + tid);
+            }
+            uint2 *qpush = queue + (qin ^ 1u) * QCAP;
             uint32_t *qpush_cnt = qcnt + (qin ^ 1u);
             // ---- read: one look per entry
+            if (!hashed) {
 #pragma unroll
-            for (int j = 0; j < R; ++j) {
-                uint32_t bk, home;
-                bool mine;
-                if (!hashed) {
+                for (int j = 0; j < R; ++j) {
                     const uint32_t x = id[j] - lo;
                     // class test: drops other classes, IDs >= N and kIdNone (lo + span <= N); a
                     // pre-partitioned bucket holds only this class, so there it drops just the padding
-                    mine = x < span;
-                    bk = __umulhi(x, bmul);
-                    home = (x << 2) & 12u;
-                } else {
-                    const uint32_t x = id[j];
-                    mine = (uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part);
-                    const uint32_t h = hash_of(x);
-                    bk = __umulhi(h, nb);                      // the high bits of h
-                    home = (h << 2) & 12u;                     // the low bits
+                    const bool mine = x < span;
+                    if (!mine) id[j] = kIdNone;
+                    t[j] = look(id[j], mine ? tbl + (__umulhi(x, bmul) << BSH) : none_addr, (x << 2) & (4u * BS - 4u));
                 }
-                if (!mine) id[j] = kIdNone;
-                t[j] = look(id[j], mine ? tbl + (bk << 4) : none_addr, home);
+            } else {
+#pragma unroll
+                for (int j = 0; j < R; ++j) {
+                    const uint32_t x = id[j];
+                    const bool mine = (uint64_t)x < p.N && (S == 1 || __umulhi(hash_round1(x), S) == part);
+                    const uint32_t h = hash_of(x);
+                    if (!mine) id[j] = kIdNone;
+                    // bucket from the high bits of h, home slot from the low bits
+                    t[j] = look(id[j], mine ? tbl + (__umulhi(h, nb) << BSH) : none_addr, (h << 2) & (4u * BS - 4u));
+                }
             }
-            uint32_t aq = none_addr;                           // the bucket the queued entry looks at
-            {
+            uint32_t aq[NQ];                                   // the buckets the queued entries look at
+#pragma unroll
+            for (int i = 0; i < NQ; ++i) {
                 uint32_t home = 0;
-                if (tid < qn) {
-                    const uint2 e = queue[qin * T + tid];
-                    id[R] = e.x; aq = e.y;
+                aq[i] = none_addr;
+                id[R + i] = kIdNone;
+                if (tid + i * T < qn) {
+                    const uint2 e = queue[qin * QCAP + tid + i * T];
+                    id[R + i] = e.x; aq[i] = e.y;
                     home = home_of(e.x);
                 }
-                t[R] = look(id[R], aq, home);
+                t[R + i] = look(id[R + i], aq[i], home);
             }
             uint32_t all = id[0];
 #pragma unroll
@@ -681,14 +713,19 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
                 // whose bucket was full (next bucket) go to the queue the next batch reads; an entry that is done
                 // reads kEmpty == its id from the empty bucket.  A full queue (IDs chosen to collide) raises
                 // misc[5]; the ID then stays with its thread and is placed right after this batch.
+                uint32_t lost = 0;
 #pragma unroll
-                for (int j = 0; j < NE; ++j) {
-                    const uint32_t cur = lds_u32(t[j]);
-                    if (cur != id[j]) {
-                        if (t[j] == none_addr) t[j] = next_bucket(j < R ? bucket_of(id[j]) : aq);
-                        const uint32_t pos = atomicAdd(qpush_cnt, 1u);
-                        if (pos < (uint32_t)T) qpush[pos] = make_uint2(id[j], t[j] & ~15u);
+                for (int j = 0; j < NE; ++j)
+                    if (lds_u32(t[j]) != id[j]) lost |= 1u << j;
+                if (lost) {                                    // one reservation per thread: no chain of atomics
+                    uint32_t pos = atomicAdd(qpush_cnt, (uint32_t)__popc(lost));
+#pragma unroll
+                    for (int j = 0; j < NE; ++j) {
+                        if (!(lost >> j & 1u)) continue;
+                        if (t[j] == none_addr) t[j] = next_bucket(j < R ? bucket_of(id[j]) : aq[j < R ? 0 : j - R]);
+                        if (pos < QCAP) qpush[pos] = make_uint2(id[j], t[j] & kBucketMask);
                         else { misc[5] = 1; keep |= 1u << j; }
+                        ++pos;
                     }
                 }
             }
@@ -700,22 +737,27 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
             }
             qin ^= 1u;                                         // the queue just filled is the next batch's input
             qn = qcnt[qin];
-            if (qn > (uint32_t)T) qn = T;
+            if (qn > QCAP) qn = QCAP;
         }
         if (qn) {                                              // list exhausted: place what the queue still holds
-            uint32_t id[1] = {kIdNone}, t[1] = {none_addr};
-            if (tid < qn) {
-                const uint2 e = queue[qin * T + tid];
-                id[0] = e.x; t[0] = e.y;
+            uint32_t id[NQ], t[NQ], keep = 0;
+#pragma unroll
+            for (int i = 0; i < NQ; ++i) {
+                id[i] = kIdNone; t[i] = none_addr;
+                if (tid + i * T < qn) {
+                    const uint2 e = queue[qin * QCAP + tid + i * T];
+                    id[i] = e.x; t[i] = e.y; keep |= 1u << i;
+                }
             }
-            place_kept(id, t, tid < qn ? 1u : 0u);
+            place_kept(id, t, keep);
         }
 
         // compact the table in bucket order: count per warp range, scan, write
         {
-            const uint32_t chunk = ((nb + T - 1) / T) * 32;   // buckets per warp, multiple of 32
-            const uint32_t v0 = warp * chunk < nb ? warp * chunk : nb;
-            const uint32_t v1 = v0 + chunk < nb ? v0 + chunk : nb;
+            const uint32_t n4 = nb * BS / 4;                   // the table as groups of 4 slots
+            const uint32_t chunk = ((n4 + 2 * T - 1) / (2 * T)) * 64;   // groups per warp, multiple of 64
+            const uint32_t v0 = warp * chunk < n4 ? warp * chunk : n4;
+            const uint32_t v1 = v0 + chunk < n4 ? v0 + chunk : n4;
             uint32_t c = 0;
             for (uint32_t v = v0 + lane; v < v1; v += 32) {
                 const uint4 w = lds_u128(tbl + (v << 4));
@@ -738,21 +780,33 @@ __global__ void __launch_bounds__(T, 1024 / T) dedup_kernel(const DedupParams p)
                 if (lane == 31) misc[0] = incl ? atomicAdd(p.uniq_counts + b, incl) : 0u;
             }
             __syncthreads();
-            // one bucket per lane and step: the lane's distinct IDs go out side by side at the warp's running
-            // position plus the count of the lanes below (three ballots on the bits of the lane's count, 0..4)
+            // eight adjacent slots per lane and step: the lane's distinct IDs (0..8) go out side by side at the
+            // warp's running position plus the counts of the lanes below (a shuffle scan)
             uint32_t *out = p.uniq_ids + off0 + misc[0] + wsum[warp];
-            for (uint32_t vb = v0; vb < v1; vb += 32) {
-                const uint32_t v = vb + lane;
-                const uint4 w = lds_u128(v < v1 ? tbl + (v << 4) : none_addr);
-                const uint32_t px = w.x != kEmpty, py = px + (w.y != kEmpty), pz = py + (w.z != kEmpty), n = pz + (w.w != kEmpty);
-                const uint32_t b0 = __ballot_sync(0xffffffffu, n & 1u), b1 = __ballot_sync(0xffffffffu, n & 2u);
-                const uint32_t b2 = __ballot_sync(0xffffffffu, n & 4u);
-                uint32_t *o = out + (__popc(b0 & lt_mask) + 2 * __popc(b1 & lt_mask) + 4 * __popc(b2 & lt_mask));
-                if (w.x != kEmpty) o[0] = w.x;
-                if (w.y != kEmpty) o[px] = w.y;
-                if (w.z != kEmpty) o[py] = w.z;
-                if (w.w != kEmpty) o[pz] = w.w;
-                out += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
+            for (uint32_t vb = v0; vb < v1; vb += 64) {
+                const uint32_t v = vb + 2 * lane;
+                const uint4 w0 = lds_u128(v < v1 ? tbl + (v << 4) : none_addr);
+                const uint4 w1 = lds_u128(v + 1 < v1 ? tbl + (v << 4) + 16 : none_addr);
+                if (v < v1) sts_u128(tbl + (v << 4), make_uint4(kEmpty, kEmpty, kEmpty, kEmpty));       // empty for the next pass
+                if (v + 1 < v1) sts_u128(tbl + (v << 4) + 16, make_uint4(kEmpty, kEmpty, kEmpty, kEmpty));
+                const uint32_t p1 = w0.x != kEmpty, p2 = p1 + (w0.y != kEmpty), p3 = p2 + (w0.z != kEmpty), p4 = p3 + (w0.w != kEmpty);
+                const uint32_t p5 = p4 + (w1.x != kEmpty), p6 = p5 + (w1.y != kEmpty), p7 = p6 + (w1.z != kEmpty), n = p7 + (w1.w != kEmpty);
+                uint32_t incl = n;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += u;
+                }
+                uint32_t *o = out + (incl - n);
+                if (w0.x != kEmpty) o[0] = w0.x;
+                if (w0.y != kEmpty) o[p1] = w0.y;
+                if (w0.z != kEmpty) o[p2] = w0.z;
+                if (w0.w != kEmpty) o[p3] = w0.w;
+                if (w1.x != kEmpty) o[p4] = w1.x;
+                if (w1.y != kEmpty) o[p5] = w1.y;
+                if (w1.z != kEmpty) o[p6] = w1.z;
+                if (w1.w != kEmpty) o[p7] = w1.w;
+                out += __shfl_sync(0xffffffffu, incl, 31);
             }
         }
     }
