@@ -149,6 +149,194 @@ def rank_seed(base_seed: int, rank: int) -> int:
     return base_seed + rank
 
 
+def traffic_from_profiles(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of `kernel` per launch at this workload, from the ncu capture
+    committed as profiles/r2_traffic.json (written from the ncu CSV named there); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    try:
+        t = json.load(open(p))
+        return int(t["workloads"][workload][kernel]), f"profiles/r2_traffic.json ({t.get('source', 'ncu')})"
+    except Exception:
+        return None, None
+
+
+def gather_ceiling(fann, ix, w, dev, nq_groups: int = 4):
+    """MEASUREMENT ONLY (include/fann_probe.h, built into its own libfann_probe.so): how fast this part reads the
+    code rows the scan kernel reads, in the scan kernel's own order and launch shape (one 512-thread CTA per SM,
+    each sweeping one query's distinct list as the dedup kernel leaves it), with none of its arithmetic.  The
+    distinct lists come from fann_dedup_only on the first queries of the timed batch.  Returns rows/s of the
+    scan kernel's fill path (cp.async ring), of the sm_100 TMA gather4 flavour and of the same rows shuffled."""
+    import ctypes as C
+    import torch
+    from paper_2409_16576_b200.build import build_probe
+    lib = C.CDLL(build_probe())
+    lib.fann_probe_gather.restype = C.c_int
+    lib.fann_probe_gather.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p,
+                                      C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.fann_probe_last_error.restype = C.c_char_p
+    info = ix.info()
+    sms, row_bytes, N = info["num_sms"], info["row_bytes"], info["N"]
+    nq = min(w.cfg.B, nq_groups * sms) // sms * sms
+    if nq == 0:
+        return None
+    off = w.cand_offsets[: nq + 1]
+    total = int(off[-1])
+    uniq, counts = ix.dedup_only(off, w.cand_ids[:total], total)
+    rps = 2048 // row_bytes                                   # rows per ring stage
+    unit = 16 * rps                                           # rows one CTA consumes per stage step
+    flats, shuffled = [], []
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(7)
+    for g in range(nq // sms):
+        c = counts[g * sms:(g + 1) * sms].long()
+        L = int(c.min()) // unit * unit
+        if L == 0:
+            continue
+        starts = off[g * sms:(g + 1) * sms]
+        idx = starts[:, None] + torch.arange(L, device=dev)[None, :]
+        q = uniq[idx]                                         # [sms, L]: every CTA's list, in the dedup's order
+        flats.append(q.view(sms, L // unit, 16, rps).permute(1, 0, 2, 3).reshape(-1))
+        perm = torch.argsort(torch.rand((sms, L), device=dev, generator=gen), dim=1)
+        shuffled.append(torch.gather(q, 1, perm).view(sms, L // unit, 16, rps).permute(1, 0, 2, 3).reshape(-1))
+    if not flats:
+        return None
+    own, rnd = torch.cat(flats).contiguous(), torch.cat(shuffled).contiguous()
+    sink = torch.zeros(4, dtype=torch.int32, device=dev)
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def rate(ids, flavor):
+        best = None
+        for it in range(4):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            rc = lib.fann_probe_gather(info["codes_device_ptr"], row_bytes, N, ids.data_ptr(), ids.numel(),
+                                       sink.data_ptr(), flavor, 1, stream)
+            b.record()
+            b.synchronize()
+            if rc != 0:
+                return None
+            if it:
+                t = a.elapsed_time(b)
+                best = t if best is None else min(best, t)
+        return ids.numel() / (best * 1e-3)
+
+    return {"rows": int(own.numel()), "queries": nq,
+            "own_order_cp_async_ring": rate(own, 3), "own_order_tma_gather4": rate(own, 4),
+            "shuffled_cp_async_ring": rate(rnd, 3)}
+
+
+def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=False, sample_clocks=False):
+    """Generate the workload, load it, warm up, time K steps of fann_build_lut + fann_dedup_scan_topk with
+    everything resident in HBM.  Returns (result dict, live objects for the legs that follow)."""
+    import numpy as np
+    import torch
+    from workloads import DEFAULT_SEED, make_workload
+    t_gen = time.time()
+    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev, keep_lists=keep_lists)   # each replica: its own batch
+    torch.cuda.synchronize()
+    t_gen = time.time() - t_gen
+    B, k, M, dsub = cfg.B, cfg.k, cfg.M, cfg.dsub
+    total = int(w.cand_ids.numel())
+
+    ix = fann.FannIndex(local_rank)
+    ix.load_codes(w.codes)
+    lut = torch.empty((B, M, 256), dtype=torch.float32, device=dev)
+    out = (torch.empty((B, k), dtype=torch.int32, device=dev), torch.empty((B, k), dtype=torch.float32, device=dev),
+           torch.empty(B, dtype=torch.int32, device=dev), torch.empty(B, dtype=torch.int32, device=dev))
+    ws = ix.workspace(B, total, k)
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step():
+        fann.fann_build_lut(ix.handle, w.queries, B, w.codebooks, dsub, lut, stream)
+        fann.fann_dedup_scan_topk(ix.handle, lut, B, w.cand_offsets, w.cand_ids, total, k,
+                                  out[0], out[1], out[2], out[3], ws, ws.numel(), stream)
+
+    # working set per step vs L2: flush between timed iterations when it could stay resident
+    flush = None
+    if total * 4 + B * M * 1024 + total * M < 4 * L2_BYTES:
+        flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    fann.fann_workspace_status(ix.handle, ws, stream)
+    U_total = int(out[3].sum().item())
+
+    fann.fann_set_timing(ix.handle, True)
+    launches0 = ix.info()["kernel_launches"]
+    sampler = ClockSampler(local_rank) if sample_clocks else None
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern = {}
+    barrier()
+    t0 = time.time()
+    for i in range(args.steps):
+        if flush is not None:
+            flush.fill_(i & 0xFF)
+        ev[i][0].record()
+        step()
+        ev[i][1].record()
+        ev[i][1].synchronize()
+        for kk, v in fann.fann_last_timing(ix.handle).items():
+            kern.setdefault(kk, []).append(v)
+    barrier()
+    t1 = time.time()
+    fann.fann_workspace_status(ix.handle, ws, stream)               # raises if any timed step overflowed a table
+    launches = ix.info()["kernel_launches"] - launches0
+    fann.fann_set_timing(ix.handle, False)
+    total_ms = float(sum(a.elapsed_time(b) for a, b in ev))
+    clocks = sampler.stop(t0, t1) if sampler else None
+    total_ms, U_all, C_all = aggregate_over_ranks(total_ms, U_total, total, device=dev)
+    ms_per_step = total_ms / args.steps
+
+    # ---- roofline of the dominant kernel (scan: code-row gather + ADC + top-k), DESIGN.md 7
+    peak, peak_src = measured_peak_gbs()
+    # the scan kernel's algorithmic bytes: code rows + the distinct IDs it reads + tables + outputs
+    algo_bytes = M * U_total + 4 * U_total + 1024 * M * B + 8 * k * B
+    # the whole step (SURVEY.md 8(d)): + candidate IDs read by the dedup stage + tables written
+    path_bytes = algo_bytes + 4 * total + 1024 * M * B
+    scan_ms = float(np.mean(kern["scan_ms"]))
+    achieved = algo_bytes / (scan_ms * 1e-3) / 1e9
+    traffic, traffic_src = traffic_from_profiles(cfg.name, "scan_kernel")
+    roofline = {"bound": "hbm", "kernel": "scan_kernel", "achieved": round(achieved, 1), "peak": peak,
+                "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kernel_ms": round(scan_ms, 4),
+                "code_bytes_only_frac": round(M * U_total / (scan_ms * 1e-3) / 1e9 / peak, 4),
+                "rows_per_s": U_total / (scan_ms * 1e-3),
+                "share_of_step": round(scan_ms / ms_per_step, 4),
+                "kernels_ms": {kk: round(float(np.mean(v)), 4) for kk, v in kern.items()}}
+    res = {"ms_per_step": ms_per_step, "value": U_all / (ms_per_step * 1e-3), "U_all": U_all, "C_all": C_all,
+           "U_total": U_total, "C_total": total, "roofline": roofline, "launches": int(launches), "clocks": clocks,
+           "path_algorithmic_bytes": path_bytes, "path_hbm_frac": round(path_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4),
+           "l2": "flushed between timed steps" if flush is not None else "inputs larger than L2",
+           "gen_seconds": round(t_gen, 1), "stats": w.stats}
+    return res, {"w": w, "ix": ix, "out": out, "ws": ws, "lut": lut}
+
+
+def sample_parity(w, cfg, out, nq):
+    """GPU output of the first nq queries against the CPU oracle (bytes for integer data, the 1e-5 band else).
+    Returns (parity flag, seconds the oracle took, oracle result, distinct candidates scored)."""
+    import numpy as np
+    dt, r, units = oracle_sample(w, nq, w.codes)
+    gi = out[0][:nq].cpu().numpy().view(np.uint32)
+    gu = out[3][:nq].cpu().numpy().view(np.uint32)
+    if cfg.integer_exact:
+        parity = bool(np.array_equal(gi, r["ids"]) and np.array_equal(gu, r["uniq"]) and
+                      np.array_equal(out[1][:nq].cpu().numpy(), r["dists"]))
+    else:
+        try:                                                        # tolerance regime: oracle/parity.py check_band
+            band_check_sample(w, min(nq, 64), w.codes, out)
+            parity = bool(np.array_equal(gu, r["uniq"]))
+        except AssertionError:
+            parity = False
+    return parity, dt, r, units
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -159,6 +347,8 @@ def main():
     ap.add_argument("--cpu-queries", type=int, default=0, help="oracle sample size (0 = auto, ~10-30 s)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-ceiling", action="store_true", help="skip the gather-ceiling probe leg")
+    ap.add_argument("--no-configs", action="store_true", help="skip the block with the other large workloads")
     ap.add_argument("--id-map", default=None, choices=["feistel", "lattice"],
                     help="vector -> ID map of the generator (default: the config's, 'feistel')")
     args = ap.parse_args()
@@ -166,7 +356,7 @@ def main():
 
     import numpy as np
     import torch
-    from workloads import CONFIGS, DEFAULT_SEED, make_workload
+    from workloads import CONFIGS
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -188,89 +378,14 @@ def main():
     from paper_2409_16576_b200.build import build
     build()
 
-    t_gen = time.time()
-    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev)     # each replica: its own batch
-    torch.cuda.synchronize()
-    t_gen = time.time() - t_gen
     B, k, M, dsub = cfg.B, cfg.k, cfg.M, cfg.dsub
-    total = int(w.cand_ids.numel())
-
-    ix = fann.FannIndex(local_rank)
-    ix.load_codes(w.codes)
-    lut = torch.empty((B, M, 256), dtype=torch.float32, device=dev)
-    out = (torch.empty((B, k), dtype=torch.int32, device=dev), torch.empty((B, k), dtype=torch.float32, device=dev),
-           torch.empty(B, dtype=torch.int32, device=dev), torch.empty(B, dtype=torch.int32, device=dev))
-    ws = ix.workspace(B, total, k)
+    want_lists = not args.no_e2e and rank == 0
+    res, live = time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=want_lists,
+                                 sample_clocks=rank == 0)
+    w, ix, out = live["w"], live["ix"], live["out"]
+    total, U_total = res["C_total"], res["U_total"]
+    roofline = res["roofline"]
     stream = torch.cuda.current_stream().cuda_stream
-
-    def step():
-        fann.fann_build_lut(ix.handle, w.queries, B, w.codebooks, dsub, lut, stream)
-        fann.fann_dedup_scan_topk(ix.handle, lut, B, w.cand_offsets, w.cand_ids, total, k,
-                                  out[0], out[1], out[2], out[3], ws, ws.numel(), stream)
-
-    # working set per step vs L2: flush between timed iterations when it could stay resident
-    U_guess_bytes = total * 4 + B * M * 1024
-    flush = None
-    if U_guess_bytes + total * M < 4 * L2_BYTES:
-        flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
-
-    def barrier():
-        if world > 1:
-            import torch.distributed as dist
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    fann.fann_workspace_status(ix.handle, ws, stream)
-    U_total = int(out[3].sum().item())
-
-    fann.fann_set_timing(ix.handle, True)
-    launches0 = ix.info()["kernel_launches"]
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern = {"lut_ms": [], "plan_ms": [], "dedup_ms": [], "scan_ms": []}
-    barrier()
-    t0 = time.time()
-    for i in range(args.steps):
-        if flush is not None:
-            flush.fill_(i & 0xFF)
-        ev[i][0].record()
-        step()
-        ev[i][1].record()
-        ev[i][1].synchronize()
-        for kk, v in fann.fann_last_timing(ix.handle).items():
-            kern[kk].append(v)
-    barrier()
-    t1 = time.time()
-    fann.fann_workspace_status(ix.handle, ws, stream)               # raises if any timed step overflowed a table
-    launches = ix.info()["kernel_launches"] - launches0
-    fann.fann_set_timing(ix.handle, False)
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    clocks = sampler.stop(t0, t1) if sampler else None
-    total_ms, U_all, C_all = aggregate_over_ranks(total_ms, U_total, total, device=dev)
-    ms_per_step = total_ms / args.steps
-    value = U_all / (ms_per_step * 1e-3)
-
-    # ---- roofline of the dominant kernel (scan: dedup + gather + ADC + local top-k)
-    peak, peak_src = measured_peak_gbs()
-    # scan kernel's own algorithmic bytes: code rows + distinct IDs + tables + outputs
-    algo_bytes = M * U_total + 4 * U_total + 1024 * M * B + 8 * k * B
-    path_bytes = algo_bytes + 4 * total + 4 * U_total                          # + dedup: IDs read, distinct IDs written
-    scan_ms = float(np.mean(kern["scan_ms"]))
-    achieved = algo_bytes / (scan_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "scan_kernel", "achieved": round(achieved, 1), "peak": peak,
-                "unit": "GB/s", "frac": round(achieved / peak, 4),
-                # dram__bytes_read+write of this kernel per gathered row, measured by ncu on this very workload
-                # (profiles/r1k_launches_u8_1b_m64.md: 50.56 GB for 7.322e8 rows of 64 bytes = 69.05 B/row); the
-                # figure is per launch like `achieved`; null for other row sizes (not captured)
-                "traffic": int(69.05 * U_total) if M > 32 else None,
-                "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kernel_ms": round(scan_ms, 4),
-                "code_bytes_only_frac": round(M * U_total / (scan_ms * 1e-3) / 1e9 / peak, 4),
-                "share_of_step": round(scan_ms / ms_per_step, 4),
-                "kernels_ms": {kk: round(float(np.mean(v)), 4) for kk, v in kern.items()}}
 
     if rank != 0:
         if world > 1:
@@ -278,78 +393,127 @@ def main():
             dist.barrier()
         return
 
-    # ---- e2e: same metric through the C ABI with HOST buffers (copies inside the timed region)
-    e2e = None
-    if not args.no_e2e:
-        need = fann.fann_search_host_scratch_bytes(ix.handle, B, dsub, total, k)
-        del ws
-        ix._ws = None
-        torch.cuda.empty_cache()
-        scratch = torch.empty(need, dtype=torch.uint8, device=dev)
-        q_h, off_h, ids_h = w.queries.cpu().pin_memory(), w.cand_offsets.cpu().pin_memory(), w.cand_ids.cpu().pin_memory()
-        oi = torch.empty((B, k), dtype=torch.int32).pin_memory()
-        od = torch.empty((B, k), dtype=torch.float32).pin_memory()
-        oc = torch.empty(B, dtype=torch.int32).pin_memory()
-
-        def host_step():
-            fann.fann_search_host(ix.handle, q_h, B, w.codebooks, dsub, off_h, ids_h, k, oi, od, oc, scratch, need, stream)
-
-        for _ in range(2):
-            host_step()
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(args.steps):
-            host_step()
-        b.record()
-        b.synchronize()
-        e_ms = a.elapsed_time(b) / args.steps
-        same = bool(np.array_equal(oi.numpy(), out[0].cpu().numpy()))
-        e2e = {"value": U_total / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": round(e_ms, 3),
-               "h2d_bytes_per_step": int(q_h.numel() * 4 + off_h.numel() * 8 + ids_h.numel() * 4),
-               "d2h_bytes_per_step": int(oi.numel() * 4 + od.numel() * 4 + oc.numel() * 4),
-               "matches_device_path": same}
-        del scratch, q_h, ids_h
+    # ---- the gather ceiling of this part for the rows of this very batch (measurement only)
+    if not args.no_ceiling:
+        try:
+            gc = gather_ceiling(fann, ix, w, dev)
+        except Exception as e:                                      # the probe must never take the bench line down
+            gc = {"error": str(e)[:200]}
+        if gc and gc.get("own_order_cp_async_ring"):
+            roofline["gather_ceiling_rows_per_s"] = gc["own_order_cp_async_ring"]
+            roofline["frac_of_gather_ceiling"] = round(roofline["rows_per_s"] / gc["own_order_cp_async_ring"], 4)
+        roofline["gather_probe"] = gc
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample, plus parity on that sample
     cpu = None
     if not args.no_cpu:
-        import oracle
         nq = args.cpu_queries
         if nq <= 0:
             dt, _, _ = oracle_sample(w, min(B, 8), w.codes)
             nq = int(max(8, min(B, 8 * 15.0 / max(dt, 1e-3))))
-        dt, r, units = oracle_sample(w, nq, w.codes)
-        gi = out[0][:nq].cpu().numpy().view(np.uint32)
-        gu = out[3][:nq].cpu().numpy().view(np.uint32)
-        if cfg.integer_exact:
-            parity = bool(np.array_equal(gi, r["ids"]) and np.array_equal(gu, r["uniq"]) and
-                          np.array_equal(out[1][:nq].cpu().numpy(), r["dists"]))
-        else:
-            try:                                                    # tolerance regime: oracle/parity.py check_band
-                band_check_sample(w, min(nq, 64), w.codes, out)
-                parity = bool(np.array_equal(gu, r["uniq"]))
-            except AssertionError:
-                parity = False
+        parity, dt, r, units = sample_parity(w, cfg, out, nq)
         cpu = {"value": units / dt, "unit": UNIT, "cores": r["threads"], "kind": "oracle",
                "sample": f"first {nq} of {B} queries of {cfg.name} ({units} distinct candidates, {dt:.2f} s)",
                "batch_qps": nq / dt, "gpu_matches_oracle_on_sample": parity}
 
+    # ---- e2e: the same metric through the C ABI with HOST buffers (copies inside the timed region).
+    # `e2e`: posting lists resident in HBM (fann_search_lists_host): queries and probed-list indices go up.
+    # `e2e_candidate_ids`: the paper's step (4) (fann_search_host): the candidate IDs themselves go up.
+    e2e, e2e_ids = None, None
+    if not args.no_e2e:
+        ref_ids = out[0].cpu().numpy()
+        del live["ws"], live["lut"]
+        ix._ws = None
+        torch.cuda.empty_cache()
+
+        def timed(fn):
+            for _ in range(2):
+                fn()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(args.steps):
+                fn()
+            b.record()
+            b.synchronize()
+            return a.elapsed_time(b) / args.steps
+
+        oi = torch.empty((B, k), dtype=torch.int32).pin_memory()
+        od = torch.empty((B, k), dtype=torch.float32).pin_memory()
+        oc = torch.empty(B, dtype=torch.int32).pin_memory()
+        q_h = w.queries.cpu().pin_memory()
+        d2h = int(oi.numel() * 4 + od.numel() * 4 + oc.numel() * 4)
+
+        ix.load_lists(w.list_offsets, w.list_ids)
+        p_h = w.probes.cpu().contiguous().pin_memory()
+        need = fann.fann_search_lists_host_scratch_bytes(ix.handle, B, dsub, cfg.nprobe, total, k)
+        scratch = torch.empty(need, dtype=torch.uint8, device=dev)
+        e_ms = timed(lambda: fann.fann_search_lists_host(ix.handle, q_h, B, w.codebooks, dsub, p_h, cfg.nprobe, total, k,
+                                                         oi, od, oc, scratch, need, stream))
+        e2e = {"value": U_total / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": round(e_ms, 3),
+               "entry": "fann_search_lists_host (posting lists resident in HBM, PAPER.md:L125 step 3 on the GPU)",
+               "h2d_bytes_per_step": int(q_h.numel() * 4 + p_h.numel() * 4), "d2h_bytes_per_step": d2h,
+               "matches_device_path": bool(np.array_equal(oi.numpy(), ref_ids))}
+        del scratch, p_h
+        torch.cuda.empty_cache()
+
+        need = fann.fann_search_host_scratch_bytes(ix.handle, B, dsub, total, k)
+        scratch = torch.empty(need, dtype=torch.uint8, device=dev)
+        off_h, ids_h = w.cand_offsets.cpu().pin_memory(), w.cand_ids.cpu().pin_memory()
+        e_ms = timed(lambda: fann.fann_search_host(ix.handle, q_h, B, w.codebooks, dsub, off_h, ids_h, k, oi, od, oc,
+                                                   scratch, need, stream))
+        e2e_ids = {"value": U_total / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": round(e_ms, 3),
+                   "entry": "fann_search_host (candidate IDs from the host, PAPER.md:L125 step 4)",
+                   "h2d_bytes_per_step": int(q_h.numel() * 4 + off_h.numel() * 8 + ids_h.numel() * 4),
+                   "d2h_bytes_per_step": d2h, "matches_device_path": bool(np.array_equal(oi.numpy(), ref_ids))}
+        del scratch, q_h, ids_h, off_h
+
+    ms_per_step = res["ms_per_step"]
+    geometry = {kk: v for kk, v in ix.info().items() if kk.startswith(("scan_", "dedup_", "table_", "row_", "chunks"))}
+    stats = res["stats"]
+
+    # ---- the other large workloads ("report both" 1B configs), same process, one after another
+    others = None
+    if world == 1 and not args.no_configs and args.workload == DEFAULT_WORKLOAD:
+        live.clear()
+        ix.close()
+        del w, ix, out
+        torch.cuda.empty_cache()
+        others = []
+        for name in ("i8_1b_m25", "f32_100m_m48", "u8_10m_m32"):
+            c2 = CONFIGS[name]
+            if args.id_map:
+                c2 = c2.scaled(id_map=args.id_map)
+            r2, l2 = time_device_path(fann, c2, args, rank, local_rank, world, dev)
+            entry = {"workload": name, "N": c2.N, "M": c2.M, "B": c2.B, "nprobe": c2.nprobe, "k": c2.k,
+                     "ms_per_step": round(r2["ms_per_step"], 4), "value": r2["value"], "unit": UNIT,
+                     "batch_qps": c2.B / (r2["ms_per_step"] * 1e-3), "C_total": r2["C_total"], "U_total": r2["U_total"],
+                     "l2": r2["l2"], "roofline": r2["roofline"]}
+            if not args.no_cpu:
+                par, dt, _, units = sample_parity(l2["w"], c2, l2["out"], min(c2.B, 48))
+                entry["gpu_matches_oracle_on_sample"] = par
+                entry["oracle_sample"] = f"first {min(c2.B, 48)} queries, {units} distinct candidates, {dt:.2f} s"
+            others.append(entry)
+            l2["ix"].close()
+            l2.clear()
+            del l2
+            torch.cuda.empty_cache()
+
     line = {
-        "path_algorithmic_bytes": path_bytes, "path_hbm_frac": round(path_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4),
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "path_algorithmic_bytes": res["path_algorithmic_bytes"], "path_hbm_frac": res["path_hbm_frac"],
+        "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "N": cfg.N, "d": cfg.d, "M": M, "B": B, "nprobe": cfg.nprobe, "k": k,
                    "id_map": cfg.id_map, "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
-                   "l2": "flushed between timed steps" if flush is not None else "inputs larger than L2",
-                   "C_total": total, "U_total": U_total, "distinct_fraction": round(U_total / max(total, 1), 4),
-                   "C_mean": w.stats["C_mean"], "C_max": w.stats["C_max"], "gen_seconds": round(t_gen, 1)},
+                   "l2": res["l2"], "C_total": total, "U_total": U_total,
+                   "distinct_fraction": round(U_total / max(total, 1), 4),
+                   "C_mean": stats["C_mean"], "C_max": stats["C_max"], "gen_seconds": res["gen_seconds"]},
         "batch_qps": B * world / (ms_per_step * 1e-3),
-        "input_ids_per_s": C_all / (ms_per_step * 1e-3),
-        "hbm_frac_nominal_8TBs": round(achieved / 8000.0, 4),
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
-        "clocks": clocks, "geometry": {kk: v for kk, v in ix.info().items() if kk.startswith(("scan_", "dedup_", "table_", "row_", "chunks"))},
+        "input_ids_per_s": res["C_all"] / (ms_per_step * 1e-3),
+        "hbm_frac_nominal_8TBs": round(roofline["achieved"] / 8000.0, 4),
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_candidate_ids": e2e_ids,
+        "gpu_launches": res["launches"], "clocks": res["clocks"], "geometry": geometry, "configs": others,
     }
     print(json.dumps(line))
     if world > 1:

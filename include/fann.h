@@ -334,14 +334,15 @@ int fann_get_info(const fann_index *ix, fann_info *out);
  * fann_build_lut / fann_dedup_scan_topk records CUDA events around its kernels on
  * the stream each kernel is launched on.  fann_last_timing synchronises on the last
  * of those events and returns, in milliseconds, the duration of the most recent
- * lookup-table kernel and plan kernel and the summed durations of the dedup
- * launches and of the scan launches (gather + ADC + top-k) of the most recent call;
- * a value is -1 if that kernel has not run since timing was enabled.  dedup_ms covers
- * the partition and the dedup kernels (with FANN_CHUNKS > 1 the partition kernels run on
- * a second stream under the scans and are not in it).  Any pointer may be NULL.
+ * lookup-table kernel, plan kernels and partition kernel and the summed durations of the
+ * dedup launches and of the scan launches (gather + ADC + top-k) of the most recent call;
+ * a value is -1 if that kernel has not run since timing was enabled (with FANN_CHUNKS > 1
+ * the partition kernels run on a second stream under the scans and are not timed).  Any
+ * pointer may be NULL.
  */
 int fann_set_timing(fann_index *ix, int enable);
-int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup_ms, float *scan_ms);
+int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *partition_ms, float *dedup_ms,
+                     float *scan_ms);
 
 #ifdef __cplusplus
 }

@@ -80,7 +80,7 @@ def load_library():
         "fann_page_reads": (i, [p, p, u32, u32, u32, p, p, p, p, p, p]),
         "fann_get_info": (i, [p, C.POINTER(_Info)]),
         "fann_set_timing": (i, [p, i]),
-        "fann_last_timing": (i, [p] + [C.POINTER(C.c_float)] * 4),
+        "fann_last_timing": (i, [p] + [C.POINTER(C.c_float)] * 5),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -254,9 +254,9 @@ def fann_set_timing(ix, enable: bool) -> None:
 
 
 def fann_last_timing(ix) -> dict:
-    v = [C.c_float(-1.0) for _ in range(4)]
+    v = [C.c_float(-1.0) for _ in range(5)]
     _check(load_library().fann_last_timing(ix, *[C.byref(x) for x in v]))
-    return dict(zip(("lut_ms", "plan_ms", "dedup_ms", "scan_ms"), (float(x.value) for x in v)))
+    return dict(zip(("lut_ms", "plan_ms", "partition_ms", "dedup_ms", "scan_ms"), (float(x.value) for x in v)))
 
 
 # ---- convenience wrapper (torch for device memory and streams only) ----------

@@ -58,8 +58,8 @@ struct fann_index {
     // optional per-kernel timing (benchmarks; timed calls are serialised by `timing_mu`)
     std::mutex timing_mu;
     std::atomic<bool> timing{false};
-    cudaEvent_t ev_lut[2] = {}, ev_plan[2] = {}, ev_dedup[kMaxChunks][2] = {}, ev_scan[kMaxChunks][2] = {};
-    bool have_lut = false, have_scan = false;
+    cudaEvent_t ev_lut[2] = {}, ev_plan[2] = {}, ev_part[2] = {}, ev_dedup[kMaxChunks][2] = {}, ev_scan[kMaxChunks][2] = {};
+    bool have_lut = false, have_scan = false, have_part = false;
     uint32_t timed_chunks = 0;
     bool timed_scan = false;
 };
@@ -249,6 +249,7 @@ extern "C" void fann_destroy(fann_index *ix)
     for (CallCtx *c : ix->ctx_pool) destroy_ctx(c);
     for (auto &e : ix->ev_lut) if (e) cudaEventDestroy(e);
     for (auto &e : ix->ev_plan) if (e) cudaEventDestroy(e);
+    for (auto &e : ix->ev_part) if (e) cudaEventDestroy(e);
     for (auto &c : ix->ev_dedup) for (auto &e : c) if (e) cudaEventDestroy(e);
     for (auto &c : ix->ev_scan) for (auto &e : c) if (e) cudaEventDestroy(e);
     delete ix;
@@ -506,13 +507,15 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     for (uint32_t c = 0; c < chunks; ++c) {
         const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
         if (overlap) CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_done[c], 0));
-        if (timing) cudaEventRecord(ix->ev_dedup[c][0], stream);
         if (!overlap && ix->partition && c == 0) {
             pp.q_begin = 0;
+            if (timing) cudaEventRecord(ix->ev_part[0], stream);
             partition_kernel<<<B, kPartThreads, 0, stream>>>(pp);
+            if (timing) { cudaEventRecord(ix->ev_part[1], stream); ix->have_part = true; }
             ix->launches++;
             CUDA_TRY(cudaGetLastError());
         }
+        if (timing) cudaEventRecord(ix->ev_dedup[c][0], stream);
         dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
         if (g.dedup_threads == 512) dedup_kernel<512, 8><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
         else dedup_kernel<1024, 8><<<ix->num_sms, 1024, g.dedup_smem, stream>>>(dp);
@@ -987,22 +990,25 @@ extern "C" int fann_set_timing(fann_index *ix, int enable)
     if (enable) {
         for (auto &e : ix->ev_lut) if (!e) CUDA_TRY(cudaEventCreate(&e));
         for (auto &e : ix->ev_plan) if (!e) CUDA_TRY(cudaEventCreate(&e));
+        for (auto &e : ix->ev_part) if (!e) CUDA_TRY(cudaEventCreate(&e));
         for (auto &c : ix->ev_dedup) for (auto &e : c) if (!e) CUDA_TRY(cudaEventCreate(&e));
         for (auto &c : ix->ev_scan) for (auto &e : c) if (!e) CUDA_TRY(cudaEventCreate(&e));
     }
     ix->timing.store(enable != 0);
-    ix->have_lut = ix->have_scan = false;
+    ix->have_lut = ix->have_scan = ix->have_part = false;
     ix->timed_chunks = 0; ix->timed_scan = false;
     return FANN_OK;
 }
 
-extern "C" int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *dedup_ms, float *scan_ms)
+extern "C" int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, float *partition_ms, float *dedup_ms,
+                                float *scan_ms)
 {
     if (!ix) return fail(FANN_EINVAL, "fann_last_timing: NULL index");
     DeviceGuard guard(ix->device);
     std::lock_guard<std::mutex> tl(ix->timing_mu);
-    float v[4] = {-1.f, -1.f, -1.f, -1.f};
+    float v[5] = {-1.f, -1.f, -1.f, -1.f, -1.f};
     if (ix->have_lut) { CUDA_TRY(cudaEventSynchronize(ix->ev_lut[1])); CUDA_TRY(cudaEventElapsedTime(&v[0], ix->ev_lut[0], ix->ev_lut[1])); }
+    if (ix->have_part) { CUDA_TRY(cudaEventSynchronize(ix->ev_part[1])); CUDA_TRY(cudaEventElapsedTime(&v[4], ix->ev_part[0], ix->ev_part[1])); }
     if (ix->have_scan && ix->timed_chunks) {
         CUDA_TRY(cudaEventSynchronize(ix->ev_plan[1]));
         CUDA_TRY(cudaEventElapsedTime(&v[1], ix->ev_plan[0], ix->ev_plan[1]));
@@ -1025,6 +1031,7 @@ extern "C" int fann_last_timing(fann_index *ix, float *lut_ms, float *plan_ms, f
     }
     if (lut_ms) *lut_ms = v[0];
     if (plan_ms) *plan_ms = v[1];
+    if (partition_ms) *partition_ms = v[4];
     if (dedup_ms) *dedup_ms = v[2];
     if (scan_ms) *scan_ms = v[3];
     return FANN_OK;

@@ -500,7 +500,6 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
     const uint32_t tbl = (uint32_t)__cvta_generic_to_shared(table);
     const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 16);   // a bucket that always holds 4 x kEmpty
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t first = p.item_start[p.q_begin], last = p.item_start[p.q_end];
 
     // Thread 0 takes the next (query, partition) item off the work counter and does its 64-bit divisions (table
