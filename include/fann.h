@@ -250,6 +250,50 @@ int fann_search_lists_host(fann_index *ix, const float *queries_h, uint32_t B,
                            void *device_scratch, size_t scratch_bytes, void *stream);
 
 /*
+ * NEXT-3 -- low-latency small-batch serving, PAPER.md:L204-L208 (section 5): "each CPU thread
+ * handles an individual query" and a "contention-free GPU memory manager": the HBM left after
+ * the codes is cut into fixed blocks, a block is handed to a query and recycled.
+ *
+ * fann_pool_create cuts one HBM allocation into n_blocks blocks, each large enough for one
+ * call of up to max_B queries with up to max_cands candidate IDs in total and k <= k_max
+ * (max_nprobe > 0 also sizes the blocks for the posting-list form).  Every block owns a CUDA
+ * stream.  fann_pool_destroy waits for the blocks' streams and frees everything.
+ *
+ * fann_search_small / fann_search_small_lists: the whole path for one small batch from HOST
+ * buffers, as fann_search_host / fann_search_lists_host, on a block of the pool and the
+ * block's stream: take a free block (waiting while all are in use), copy up, run, copy the
+ * results back, synchronise the block's stream, give the block back.  Any number of host
+ * threads may call concurrently on one index and one pool; calls share no workspace, stream
+ * or event.  A batch of fewer queries than half the SMs is scanned by several CTAs per query
+ * (each on a slice of the query's distinct list, merged on the device), so that one query
+ * does not wait on one SM; results are the same bytes as the batched entry points give.
+ * Errors: EINVAL (NULL, a pool of another index, B / k / dsub / nprobe outside what the pool
+ * was created for), EWORKSPACE (more candidate IDs than a block holds), and what the batched
+ * entry points return.
+ */
+typedef struct fann_pool fann_pool;
+typedef struct fann_pool_info {
+    uint64_t block_bytes;        /* HBM per block                                              */
+    uint64_t calls;              /* blocks handed out so far                                   */
+    uint64_t waits;              /* calls that found every block in use and had to wait        */
+    uint32_t n_blocks, in_use;   /* blocks of the pool; blocks handed out right now            */
+    uint32_t high_water;         /* most blocks in use at the same time so far                 */
+    uint32_t reserved;
+} fann_pool_info;
+int fann_pool_create(fann_index *ix, uint32_t n_blocks, uint32_t max_B, uint64_t max_cands, uint32_t dsub,
+                     uint32_t max_nprobe, uint32_t k_max, fann_pool **out);
+void fann_pool_destroy(fann_pool *pool);
+int fann_pool_stats(fann_pool *pool, fann_pool_info *out);
+int fann_search_small(fann_index *ix, fann_pool *pool, const float *queries_h, uint32_t B,
+                      const float *codebooks_d, uint32_t dsub,
+                      const int64_t *cand_offsets_h, const uint32_t *cand_ids_h, uint32_t k,
+                      uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h);
+int fann_search_small_lists(fann_index *ix, fann_pool *pool, const float *queries_h, uint32_t B,
+                            const float *codebooks_d, uint32_t dsub,
+                            const uint32_t *probes_h, uint32_t nprobe, uint32_t k,
+                            uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h);
+
+/*
  * NEXT-1 -- heuristic re-ranking, PAPER.md:L164-L182 (section 4.2, Eq. 3, Algorithm 1), with the
  * raw vectors in HBM instead of on SSD (the configurations whose raw vectors fit).
  *

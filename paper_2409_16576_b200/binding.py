@@ -40,6 +40,11 @@ class _Info(C.Structure):
                 ("reserved", C.c_uint32), ("kernel_launches", C.c_uint64), ("codes_device_ptr", C.c_uint64)]
 
 
+class _PoolInfo(C.Structure):
+    _fields_ = [("block_bytes", C.c_uint64), ("calls", C.c_uint64), ("waits", C.c_uint64), ("n_blocks", C.c_uint32),
+                ("in_use", C.c_uint32), ("high_water", C.c_uint32), ("reserved", C.c_uint32)]
+
+
 def library_path() -> str:
     return _LIB_PATH
 
@@ -74,6 +79,11 @@ def load_library():
         "fann_search_lists_status": (i, [p, p, u32, u64, u32, C.POINTER(u64), p]),
         "fann_search_lists_host_scratch_bytes": (sz, [p, u32, u32, u32, u64, u32]),
         "fann_search_lists_host": (i, [p, p, u32, p, u32, p, u32, u64, u32, p, p, p, p, sz, p]),
+        "fann_pool_create": (i, [p, u32, u32, u64, u32, u32, u32, C.POINTER(p)]),
+        "fann_pool_destroy": (None, [p]),
+        "fann_pool_stats": (i, [p, C.POINTER(_PoolInfo)]),
+        "fann_search_small": (i, [p, p, p, u32, p, u32, p, p, u32, p, p, p]),
+        "fann_search_small_lists": (i, [p, p, p, u32, p, u32, p, u32, u32, p, p, p]),
         "fann_load_vectors": (i, [p, p, u64, u64, u64, u32, i, i, p]),
         "fann_rerank": (i, [p, p, u32, p, u32, u32, u32, C.c_float, u32, p, p, p, p, p, p]),
         "fann_load_page_table": (i, [p, p, u64, u64, i, p]),
@@ -218,6 +228,37 @@ def fann_search_lists_host(ix, queries_h, B, codebooks_d, dsub, probes_h, nprobe
     _check(load_library().fann_search_lists_host(ix, _addr(queries_h), B, _addr(codebooks_d), dsub, _addr(probes_h),
                                                  nprobe, max_total_cands, k, _addr(out_ids_h), _addr(out_dists_h),
                                                  _addr(out_counts_h), _addr(device_scratch), scratch_bytes, stream))
+
+
+def fann_pool_create(ix, n_blocks, max_B, max_cands, dsub, max_nprobe, k_max) -> int:
+    h = C.c_void_p()
+    _check(load_library().fann_pool_create(ix, n_blocks, max_B, max_cands, dsub, max_nprobe, k_max, C.byref(h)))
+    return h.value
+
+
+def fann_pool_destroy(pool) -> None:
+    load_library().fann_pool_destroy(pool)
+
+
+def fann_pool_stats(pool) -> dict:
+    info = _PoolInfo()
+    _check(load_library().fann_pool_stats(pool, C.byref(info)))
+    return {name: int(getattr(info, name)) for name, _ in _PoolInfo._fields_ if name != "reserved"}
+
+
+def fann_search_small(ix, pool, queries_h, B, codebooks_d, dsub, cand_offsets_h, cand_ids_h, k, out_ids_h, out_dists_h,
+                      out_counts_h) -> None:
+    """ctypes releases the GIL during the call, so Python threads really run their calls side by side."""
+    _check(load_library().fann_search_small(ix, pool, _addr(queries_h), B, _addr(codebooks_d), dsub,
+                                            _addr(cand_offsets_h), _addr(cand_ids_h), k, _addr(out_ids_h),
+                                            _addr(out_dists_h), _addr(out_counts_h)))
+
+
+def fann_search_small_lists(ix, pool, queries_h, B, codebooks_d, dsub, probes_h, nprobe, k, out_ids_h, out_dists_h,
+                            out_counts_h) -> None:
+    _check(load_library().fann_search_small_lists(ix, pool, _addr(queries_h), B, _addr(codebooks_d), dsub,
+                                                  _addr(probes_h), nprobe, k, _addr(out_ids_h), _addr(out_dists_h),
+                                                  _addr(out_counts_h)))
 
 
 def fann_load_vectors(ix, vectors, first, n, N_total, d, elem_type, src_is_device, stream=None) -> None:

@@ -5,6 +5,7 @@
 #include "fann_next.cuh"
 
 #include <atomic>
+#include <condition_variable>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -46,6 +47,7 @@ struct fann_index {
     uint32_t force_mode = 2;               // dedup placement: 0 ordered, 1 hashed, 2 decided per query (FANN_DEDUP_MODE)
     uint32_t scan_ring = 3;                // scan kernel: stages of the per-warp code-row ring, 0 = rows through registers (FANN_SCAN_RING)
     bool partition = true;                 // split lists into their dedup classes first (FANN_PARTITION=0: filter per pass)
+    bool split_scan = true;                // several scan CTAs per query when the batch is smaller than the machine (FANN_SPLIT_SCAN=0: one)
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint32_t dedup_smem_half = 0;          // same for two CTAs per SM
     uint32_t dedup_threads = 0;            // 0: chosen per call (geometry()); 1024 or 512: forced (FANN_DEDUP_THREADS)
@@ -131,12 +133,14 @@ struct CtxLease {
 struct Geom {
     uint32_t nslots_max, cap_c, dedup_smem, dedup_threads;   // dedup: table slots per CTA, candidates per partition, CTA shape
     uint32_t cap, scan_smem, ring;                   // scan: candidate-buffer keys, shared memory per CTA, ring depth
+    uint32_t parts, k;                               // scan CTAs per query (> 1 for batches smaller than the machine), k
 };
 
 // Dedup CTA shape: one 1024-thread CTA per SM with the whole shared memory as its table, or -- when the mean candidate
 // list needs two or more partitions anyway -- two 512-thread CTAs per SM with half the table each, so that one computes
 // while the other waits at a barrier (partition_kernel makes the number of partitions free: each ID is read once).
-static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t total_cands, Geom *g, uint32_t shape = 0)
+static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t total_cands, Geom *g, uint32_t shape = 0,
+                     bool allow_split = true)
 {
     g->dedup_threads = 1024; g->dedup_smem = ix->dedup_smem;
     g->nslots_max = ((g->dedup_smem - dedup_table_off(1024)) / 4) & ~3u;
@@ -150,12 +154,20 @@ static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t tota
         g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);
     }
     g->ring = ix->scan_ring;
+    // a batch of fewer queries than half the SMs: several scan CTAs per query, each on a slice of the query's
+    // distinct list, merged by merge_parts_kernel (at most 16 parts: 16 k keys fit the merge CTA's shared memory)
+    g->k = k;
+    g->parts = 1;
+    if (ix->split_scan && allow_split && 2 * B <= (uint32_t)ix->num_sms) {
+        g->parts = (uint32_t)ix->num_sms / B;
+        if (g->parts > 16) g->parts = 16;
+    }
     g->cap = (k <= 256 || g->ring) ? 4096u : 8192u;            // the ring takes the shared memory of the larger buffer
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap, g->ring);
 }
 
 struct WsLayout {
-    size_t hdr, S, mode, item_start, items, uniq_counts, part_ok, bucket_cnt, part_ids, uniq_ids, total;
+    size_t hdr, S, mode, item_start, items, uniq_counts, part_ok, bucket_cnt, part_keys, part_ids, uniq_ids, total;
     uint32_t max_items;
 };
 
@@ -172,6 +184,7 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
     w->uniq_counts = o; o = align_up(o + (size_t)B * 4, 256);
     w->part_ok = o;     o = align_up(o + (size_t)B * 4, 256);
     w->bucket_cnt = o;  o = align_up(o + (size_t)w->max_items * 4, 256);
+    w->part_keys = o;   if (g.parts > 1) o = align_up(o + (size_t)B * g.parts * g.k * 8, 256);   // partial top-k of the scan parts
     w->part_ids = o;    o = align_up(o + (size_t)total_cands * 8 + 16, 256);      // class buckets, 2 C_b per query
     w->uniq_ids = o;    if (with_uniq) o = align_up(o + (size_t)total_cands * 4 + 16, 256);
     w->total = o;
@@ -218,6 +231,7 @@ extern "C" int fann_create(fann_index **out, int device)
     CUDA_TRY((set_scan_attr<1, 4, 3>(ring_max)));
     CUDA_TRY((set_scan_attr<2, 4, 3>(ring_max)));
     CUDA_TRY((set_scan_attr<4, 2, 3>(ring_max)));
+    CUDA_TRY(cudaFuncSetAttribute(merge_parts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 8));
     int per_sm = 0;
     CUDA_TRY(cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device));
     fann_index *ix = new fann_index();
@@ -229,6 +243,7 @@ extern "C" int fann_create(fann_index **out, int device)
     if (const char *s = getenv("FANN_CHUNKS")) { int v = atoi(s); if (v >= 1 && v <= kMaxChunks) ix->chunks = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
     if (const char *s = getenv("FANN_PARTITION")) ix->partition = atoi(s) != 0;
+    if (const char *s = getenv("FANN_SPLIT_SCAN")) ix->split_scan = atoi(s) != 0;
     if (const char *s = getenv("FANN_SCAN_RING")) { int v = atoi(s); if (v == 0 || v == 3) ix->scan_ring = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_THREADS")) { int v = atoi(s); if (v == 512 || v == 1024) ix->dedup_threads = (uint32_t)v; }
     *out = ix;
@@ -424,10 +439,10 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     uint32_t k, uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
                     uint32_t *out_uniq, uint32_t *uniq_ids, uint32_t *uniq_counts,
                     void *workspace, size_t workspace_bytes, cudaStream_t stream,
-                    uint32_t shape = 0, bool keep_status = false, bool exact_total = true)
+                    uint32_t shape = 0, bool keep_status = false, bool exact_total = true, bool allow_split = true)
 {
     Geom g;
-    geometry(ix, k, B, total_cands, &g, shape);
+    geometry(ix, k, B, total_cands, &g, shape, allow_split);
     WsLayout w;
     ws_layout(B, total_cands, g, !dump, &w);
     if (!workspace || ((uintptr_t)workspace & 255) != 0)
@@ -488,6 +503,9 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
     sp.out_ids = out_ids; sp.out_dists = out_dists; sp.out_counts = out_counts; sp.out_uniq = out_uniq;
+    sp.parts = g.parts; sp.part_keys = (unsigned long long *)(ws + w.part_keys);
+    uint32_t merge_n2 = 32;
+    while (merge_n2 < g.parts * k) merge_n2 <<= 1;
     const int per_sm = dump ? 1 : scan_ctas_per_sm(ix, g.scan_smem);
 
     // With chunks > 1 the partition launches of all chunks go to the side stream at once: the partition kernel is
@@ -525,9 +543,15 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         if (dump) continue;
         sp.q_begin = qb; sp.q_end = qe; sp.counter = &hdr->scan_counter[c];
         int grid = ix->num_sms * per_sm;
-        if ((uint32_t)grid > qe - qb) grid = (int)(qe - qb);
+        if ((uint32_t)grid > (qe - qb) * g.parts) grid = (int)((qe - qb) * g.parts);
         if (timing) cudaEventRecord(ix->ev_scan[c][0], stream);
         cudaError_t e = launch_scan(ix, grid, g.scan_smem, stream, sp);
+        if (e == cudaSuccess && g.parts > 1) {
+            merge_parts_kernel<<<qe - qb, kMergeThreads, (size_t)merge_n2 * 8, stream>>>(
+                sp.part_keys, uniq_counts, qb, g.parts, k, merge_n2, out_ids, out_dists, out_counts, out_uniq);
+            ix->launches++;
+            e = cudaGetLastError();
+        }
         if (timing) cudaEventRecord(ix->ev_scan[c][1], stream);
         ix->launches++;
         if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
@@ -676,7 +700,7 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
                       (const int64_t *)(s + h.offsets) + b0, (const uint32_t *)(s + h.ids), total, k,
                       (uint32_t *)(s + h.out_ids) + (size_t)b0 * k, (float *)(s + h.out_dists) + (size_t)b0 * k,
                       (uint32_t *)(s + h.out_counts) + b0, nullptr, nullptr, nullptr,
-                      s + h.ws, h.ws_bytes, stream, g.dedup_threads, c > 0, nchunk == 1);
+                      s + h.ws, h.ws_bytes, stream, g.dedup_threads, c > 0, nchunk == 1, nchunk == 1);
         if (rc != FANN_OK) return rc;
     }
     CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
@@ -867,6 +891,137 @@ extern "C" int fann_search_lists_host(fann_index *ix, const float *queries_h, ui
     if (out_counts_h)
         CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
     return fann_search_lists_status(ix, s + h.ws, B, max_total_cands, k, nullptr, stream);   // synchronises
+}
+
+// ---------------------------------------------------------------- NEXT-3: low-latency small-batch serving
+
+// "the remaining HBM space is divided into multiple blocks ... each block is allocated to an
+// individual query ... recycled".  A pool is one HBM allocation cut into fixed blocks; a call takes a free block
+// (and the stream that belongs to it) and gives it back when its results are on the host.
+struct fann_pool {
+    fann_index *ix = nullptr;
+    char *mem = nullptr;
+    size_t block_bytes = 0;
+    uint32_t n_blocks = 0, max_B = 0, k_max = 0, dsub = 0, max_nprobe = 0;
+    uint64_t max_cands = 0;
+    std::vector<cudaStream_t> streams;
+    std::mutex mu;
+    std::condition_variable cv;
+    std::vector<uint32_t> free_blocks;
+    uint32_t in_use = 0, high_water = 0;
+    uint64_t calls = 0, waits = 0;
+};
+
+struct BlockLease {
+    fann_pool *pool;
+    uint32_t id;
+    explicit BlockLease(fann_pool *p) : pool(p)
+    {
+        std::unique_lock<std::mutex> g(p->mu);
+        if (p->free_blocks.empty()) { p->waits++; p->cv.wait(g, [&] { return !p->free_blocks.empty(); }); }
+        id = p->free_blocks.back();
+        p->free_blocks.pop_back();
+        p->in_use++; p->calls++;
+        if (p->in_use > p->high_water) p->high_water = p->in_use;
+    }
+    ~BlockLease()
+    {
+        { std::lock_guard<std::mutex> g(pool->mu); pool->free_blocks.push_back(id); pool->in_use--; }
+        pool->cv.notify_one();
+    }
+    char *mem() const { return pool->mem + (size_t)id * pool->block_bytes; }
+    cudaStream_t stream() const { return pool->streams[id]; }
+};
+
+extern "C" int fann_pool_create(fann_index *ix, uint32_t n_blocks, uint32_t max_B, uint64_t max_cands, uint32_t dsub,
+                                uint32_t max_nprobe, uint32_t k_max, fann_pool **out)
+{
+    if (!ix || !out) return fail(FANN_EINVAL, "fann_pool_create: NULL argument");
+    *out = nullptr;
+    if (!ix->codes) return fail(FANN_EINVAL, "fann_pool_create: load codes first");
+    if (n_blocks == 0 || n_blocks > 4096 || max_B == 0 || dsub == 0 || k_max == 0 || k_max > FANN_MAX_K)
+        return fail(FANN_EINVAL, "fann_pool_create: n_blocks=%u max_B=%u dsub=%u k_max=%u", n_blocks, max_B, dsub, k_max);
+    if (max_nprobe > FANN_MAX_NPROBE) return fail(FANN_EUNSUPPORTED, "fann_pool_create: max_nprobe=%u > %u", max_nprobe, FANN_MAX_NPROBE);
+    DeviceGuard guard(ix->device);
+    HostScratch h;
+    host_scratch_layout(ix, max_B, dsub, max_cands, k_max, &h);
+    size_t need = h.total;
+    if (max_nprobe) {
+        ListsHostScratch lh;
+        lists_host_layout(ix, max_B, dsub, max_nprobe, max_cands, k_max, &lh);
+        if (lh.total > need) need = lh.total;
+    }
+    // the partial top-k of the scan parts depends on the batch size of the call: at most num_sms x k keys
+    need = align_up(need + (size_t)ix->num_sms * k_max * 8 + 4096, 256);
+    fann_pool *p = new fann_pool();
+    p->ix = ix; p->block_bytes = need; p->n_blocks = n_blocks; p->max_B = max_B; p->k_max = k_max; p->dsub = dsub;
+    p->max_nprobe = max_nprobe; p->max_cands = max_cands;
+    cudaError_t e = cudaMalloc(&p->mem, need * n_blocks);
+    if (e != cudaSuccess) {
+        delete p;
+        return fail(FANN_ENOMEM, "fann_pool_create: cudaMalloc(%zu x %u): %s", need, n_blocks, cudaGetErrorString(e));
+    }
+    for (uint32_t i = 0; i < n_blocks; ++i) {
+        cudaStream_t st = nullptr;
+        if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) {
+            for (auto s2 : p->streams) cudaStreamDestroy(s2);
+            cudaFree(p->mem);
+            delete p;
+            return fail(FANN_ECUDA, "fann_pool_create: could not create stream %u", i);
+        }
+        p->streams.push_back(st);
+        p->free_blocks.push_back(n_blocks - 1 - i);
+    }
+    *out = p;
+    return FANN_OK;
+}
+
+extern "C" void fann_pool_destroy(fann_pool *p)
+{
+    if (!p) return;
+    DeviceGuard guard(p->ix->device);
+    for (auto st : p->streams) { cudaStreamSynchronize(st); cudaStreamDestroy(st); }
+    if (p->mem) cudaFree(p->mem);
+    delete p;
+}
+
+extern "C" int fann_pool_stats(fann_pool *p, fann_pool_info *out)
+{
+    if (!p || !out) return fail(FANN_EINVAL, "fann_pool_stats: NULL argument");
+    std::lock_guard<std::mutex> g(p->mu);
+    out->block_bytes = p->block_bytes; out->calls = p->calls; out->waits = p->waits;
+    out->n_blocks = p->n_blocks; out->in_use = p->in_use; out->high_water = p->high_water; out->reserved = 0;
+    return FANN_OK;
+}
+
+extern "C" int fann_search_small(fann_index *ix, fann_pool *pool, const float *queries_h, uint32_t B,
+                                 const float *codebooks_d, uint32_t dsub, const int64_t *cand_offsets_h,
+                                 const uint32_t *cand_ids_h, uint32_t k, uint32_t *out_ids_h, float *out_dists_h,
+                                 uint32_t *out_counts_h)
+{
+    if (!ix || !pool || pool->ix != ix) return fail(FANN_EINVAL, "fann_search_small: NULL index or a pool of another index");
+    if (B == 0 || B > pool->max_B || k == 0 || k > pool->k_max || dsub != pool->dsub)
+        return fail(FANN_EINVAL, "fann_search_small: B=%u (pool: %u), k=%u (pool: %u), dsub=%u (pool: %u)", B, pool->max_B, k,
+                    pool->k_max, dsub, pool->dsub);
+    if (cand_offsets_h && (cand_offsets_h[B] < 0 || (uint64_t)cand_offsets_h[B] > pool->max_cands))
+        return fail(FANN_EWORKSPACE, "fann_search_small: %lld candidate IDs, the pool's blocks hold %llu",
+                    (long long)cand_offsets_h[B], (unsigned long long)pool->max_cands);
+    BlockLease lease(pool);                                    // waits while every block is in use
+    return fann_search_host(ix, queries_h, B, codebooks_d, dsub, cand_offsets_h, cand_ids_h, k, out_ids_h, out_dists_h,
+                            out_counts_h, lease.mem(), pool->block_bytes, lease.stream());
+}
+
+extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const float *queries_h, uint32_t B,
+                                       const float *codebooks_d, uint32_t dsub, const uint32_t *probes_h, uint32_t nprobe,
+                                       uint32_t k, uint32_t *out_ids_h, float *out_dists_h, uint32_t *out_counts_h)
+{
+    if (!ix || !pool || pool->ix != ix) return fail(FANN_EINVAL, "fann_search_small_lists: NULL index or a pool of another index");
+    if (B == 0 || B > pool->max_B || k == 0 || k > pool->k_max || dsub != pool->dsub || nprobe == 0 || nprobe > pool->max_nprobe)
+        return fail(FANN_EINVAL, "fann_search_small_lists: B=%u (pool: %u), k=%u (pool: %u), dsub=%u (pool: %u), nprobe=%u (pool: %u)",
+                    B, pool->max_B, k, pool->k_max, dsub, pool->dsub, nprobe, pool->max_nprobe);
+    BlockLease lease(pool);
+    return fann_search_lists_host(ix, queries_h, B, codebooks_d, dsub, probes_h, nprobe, pool->max_cands, k, out_ids_h,
+                                  out_dists_h, out_counts_h, lease.mem(), pool->block_bytes, lease.stream());
 }
 
 // ---------------------------------------------------------------- NEXT-1: heuristic re-ranking

@@ -840,6 +840,8 @@ struct ScanParams {
     float *out_dists;                                // [B][k]
     uint32_t *out_counts;                            // [B] or NULL
     uint32_t *out_uniq;                              // [B] or NULL
+    uint32_t parts;                                  // CTAs per query: > 1 splits a query's distinct list (small batches)
+    unsigned long long *part_keys;                   // [B][parts][k] partial top-k keys, merged by merge_parts_kernel
 };
 
 // Column of sub-space m in the c-major shared-memory table.  G = 16-byte chunks (= lanes) per row.
@@ -1005,13 +1007,21 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 
     for (;;) {
         __syncthreads();                                       // previous query fully done
-        if (tid == 0) misc[2] = p.q_begin + atomicAdd(p.counter, 1u);
+        if (tid == 0) misc[2] = atomicAdd(p.counter, 1u);
         __syncthreads();
-        const uint32_t b = misc[2];
-        if (b >= p.q_end) break;
+        const uint32_t work = misc[2];                         // (query, part of its distinct list)
+        if (work >= (p.q_end - p.q_begin) * p.parts) break;
+        const uint32_t b = p.q_begin + work / p.parts, part = work % p.parts;
         const long long off0 = p.cand_offsets[b];
-        const uint32_t U = p.uniq_counts[b];
+        uint32_t U = p.uniq_counts[b];
         const uint32_t *uq = p.uniq_ids + off0;
+        if (p.parts > 1) {                                     // this CTA's slice, cut at multiples of 512 IDs
+            const uint32_t chunks = (U + 511u) >> 9;
+            const uint32_t c0 = (uint32_t)((unsigned long long)chunks * part / p.parts) << 9;
+            const uint32_t c1 = (uint32_t)((unsigned long long)chunks * (part + 1) / p.parts) << 9;
+            uq += c0;
+            U = (c1 < U ? c1 : U) - (c0 < U ? c0 : U);
+        }
 
         {   // stage the lookup table c-major; each warp writes 32 different banks per store
             constexpr uint32_t ncols = G == 4 ? 64 : 32;
@@ -1175,6 +1185,11 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
         __syncthreads();
         bitonic_sort_smem(buf, P, 2);
         const uint32_t cnt = n < p.k ? n : p.k;
+        if (p.parts > 1) {                                     // partial result: the slice's k smallest keys, padded
+            unsigned long long *pk = p.part_keys + ((size_t)b * p.parts + part) * p.k;
+            for (uint32_t i = tid; i < p.k; i += kScanThreads) pk[i] = i < cnt ? buf[i] : kKeyMax;
+            continue;
+        }
         for (uint32_t i = tid; i < p.k; i += kScanThreads) {
             const bool pad = i >= cnt;
             const unsigned long long key = pad ? kKeyMax : buf[i];
@@ -1185,6 +1200,35 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             if (p.out_counts) p.out_counts[b] = cnt;
             if (p.out_uniq) p.out_uniq[b] = U;
         }
+    }
+}
+
+// Small batches: scan_kernel ran `parts` CTAs per query, each on a slice of the query's
+// distinct list; the slices are disjoint, so the query's top-k is the k smallest of the parts' keys.  One CTA per
+// query sorts them in shared memory (n2 = power of two >= parts * k keys) and writes the outputs of step (7).
+constexpr int kMergeThreads = 512;
+__global__ void __launch_bounds__(kMergeThreads) merge_parts_kernel(const unsigned long long *__restrict__ part_keys,
+                                                                    const uint32_t *__restrict__ uniq_counts, uint32_t q_begin,
+                                                                    uint32_t parts, uint32_t k, uint32_t n2, uint32_t *out_ids,
+                                                                    float *out_dists, uint32_t *out_counts, uint32_t *out_uniq)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    unsigned long long *buf = reinterpret_cast<unsigned long long *>(smem);
+    const uint32_t b = q_begin + blockIdx.x, tid = threadIdx.x, n = parts * k;
+    const unsigned long long *src = part_keys + (size_t)b * n;
+    for (uint32_t i = tid; i < n2; i += kMergeThreads) buf[i] = i < n ? src[i] : kKeyMax;
+    __syncthreads();
+    bitonic_sort_smem(buf, n2, 2);
+    const uint32_t U = uniq_counts[b], cnt = U < k ? U : k;
+    for (uint32_t i = tid; i < k; i += kMergeThreads) {
+        const bool pad = i >= cnt;
+        const unsigned long long key = buf[i];
+        out_ids[(size_t)b * k + i] = pad ? kIdNone : (uint32_t)key;
+        out_dists[(size_t)b * k + i] = pad ? __int_as_float(0x7f800000) : __uint_as_float((uint32_t)(key >> 32));
+    }
+    if (tid == 0) {
+        if (out_counts) out_counts[b] = cnt;
+        if (out_uniq) out_uniq[b] = U;
     }
 }
 

@@ -251,11 +251,12 @@ def test_k1000_partitions_bytes(fann, w_k1000):
     {"FANN_DEDUP_MODE": "1", "FANN_PARTITION": "0"},
     {"FANN_SCAN_RING": "0"},                             # code rows through registers
     {"FANN_CHUNKS": "4"},                                # dedup of chunk i+1 on a second stream beside the scan of chunk i
+    {"FANN_SPLIT_SCAN": "0"},                            # one scan CTA per query even when the batch is smaller than the machine
 ])
 def test_every_code_path_gives_the_same_bytes(fann, w_k1000, w_i8, monkeypatch, env):
     """The library picks CTA shapes, placement and staging by itself; each alternative (also the
     fallbacks it takes on bunched IDs or refused splits) must give the oracle's bytes."""
-    for key in ("FANN_DEDUP_THREADS", "FANN_PARTITION", "FANN_DEDUP_MODE", "FANN_SCAN_RING", "FANN_CHUNKS"):
+    for key in ("FANN_DEDUP_THREADS", "FANN_PARTITION", "FANN_DEDUP_MODE", "FANN_SCAN_RING", "FANN_CHUNKS", "FANN_SPLIT_SCAN"):
         monkeypatch.delenv(key, raising=False)
     for key, val in env.items():
         monkeypatch.setenv(key, val)
