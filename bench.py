@@ -318,6 +318,58 @@ def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=F
     return res, {"w": w, "ix": ix, "out": out, "ws": ws, "lut": lut}
 
 
+def small_batch_leg(fann, ix, w, cfg, dev, ref_ids):
+    """the path one small batch at a time through the block pool
+    (fann_search_small_lists: queries and probed-list indices from HOST buffers, results back on the host).
+    Latency is the host's wall clock around the synchronous call; throughput is queries answered per second by
+    T host threads calling at the same time on one handle."""
+    import threading
+    import numpy as np
+    k, dsub, nprobe = cfg.k, cfg.dsub, cfg.nprobe
+    nq = min(cfg.B, 512)
+    per_q = int((w.cand_offsets[1:nq + 1] - w.cand_offsets[:nq]).max())
+    max_B = min(64, cfg.B)
+    pool = fann.fann_pool_create(ix.handle, 8, max_B, per_q * max_B, dsub, nprobe, k)
+    q_h = w.queries[:nq].cpu().pin_memory()
+    p_h = w.probes[:nq].cpu().contiguous().pin_memory()
+    res = {"entry": "fann_search_small_lists", "pool_blocks": 8, "timing": "host wall clock around the synchronous call"}
+    ok = True
+    for B in (1, 8, max_B):
+        oi = np.zeros((B, k), np.uint32); od = np.zeros((B, k), np.float32); oc = np.zeros(B, np.uint32)
+        ts = []
+        for it in range(24):
+            b0 = (it * B) % (nq - B + 1)
+            t0 = time.perf_counter()
+            fann.fann_search_small_lists(ix.handle, pool, q_h[b0:b0 + B], B, w.codebooks, dsub, p_h[b0:b0 + B], nprobe, k, oi, od, oc)
+            ts.append(time.perf_counter() - t0)
+            ok = ok and bool(np.array_equal(oi.view(np.int32), ref_ids[b0:b0 + B]))
+        ts = sorted(ts[4:])
+        res[f"B{B}"] = {"latency_us_p50": round(1e6 * ts[len(ts) // 2], 1), "latency_us_p90": round(1e6 * ts[int(len(ts) * 0.9)], 1),
+                        "qps_one_thread": round(B / ts[len(ts) // 2], 1)}
+    for T in (4, 8):
+        done = [0] * T
+        stop = time.perf_counter() + 0.6
+
+        def worker(t):
+            oi = np.zeros((1, k), np.uint32); od = np.zeros((1, k), np.float32); oc = np.zeros(1, np.uint32)
+            b = t
+            while time.perf_counter() < stop:
+                fann.fann_search_small_lists(ix.handle, pool, q_h[b:b + 1], 1, w.codebooks, dsub, p_h[b:b + 1], nprobe, k, oi, od, oc)
+                done[t] += 1
+                b = (b + T) % nq
+        t0 = time.perf_counter()
+        th = [threading.Thread(target=worker, args=(t,)) for t in range(T)]
+        for x in th:
+            x.start()
+        for x in th:
+            x.join()
+        res[f"threads{T}_B1_qps"] = round(sum(done) / (time.perf_counter() - t0), 1)
+    res["matches_device_path"] = ok
+    res["pool"] = fann.fann_pool_stats(pool)
+    fann.fann_pool_destroy(pool)
+    return res
+
+
 def sample_parity(w, cfg, out, nq):
     """GPU output of the first nq queries against the CPU oracle (bytes for integer data, the 1e-5 band else).
     Returns (parity flag, seconds the oracle took, oracle result, distinct candidates scored)."""
@@ -419,7 +471,7 @@ def main():
     # ---- e2e: the same metric through the C ABI with HOST buffers (copies inside the timed region).
     # `e2e`: posting lists resident in HBM (fann_search_lists_host): queries and probed-list indices go up.
     # `e2e_candidate_ids`: the paper's step (4) (fann_search_host): the candidate IDs themselves go up.
-    e2e, e2e_ids = None, None
+    e2e, e2e_ids, small = None, None, None
     if not args.no_e2e:
         ref_ids = out[0].cpu().numpy()
         del live["ws"], live["lut"]
@@ -456,6 +508,10 @@ def main():
                "matches_device_path": bool(np.array_equal(oi.numpy(), ref_ids))}
         del scratch, p_h
         torch.cuda.empty_cache()
+        try:
+            small = small_batch_leg(fann, ix, w, cfg, dev, ref_ids)
+        except Exception as e:                                      # never take the bench line down
+            small = {"error": str(e)[:200]}
 
         need = fann.fann_search_host_scratch_bytes(ix.handle, B, dsub, total, k)
         scratch = torch.empty(need, dtype=torch.uint8, device=dev)
@@ -512,7 +568,7 @@ def main():
         "batch_qps": B * world / (ms_per_step * 1e-3),
         "input_ids_per_s": res["C_all"] / (ms_per_step * 1e-3),
         "hbm_frac_nominal_8TBs": round(roofline["achieved"] / 8000.0, 4),
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_candidate_ids": e2e_ids,
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_candidate_ids": e2e_ids, "small_batch": small,
         "gpu_launches": res["launches"], "clocks": res["clocks"], "geometry": geometry, "configs": others,
     }
     print(json.dumps(line))

@@ -159,8 +159,8 @@ static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t tota
     g->k = k;
     g->parts = 1;
     if (ix->split_scan && allow_split && 2 * B <= (uint32_t)ix->num_sms) {
-        g->parts = (uint32_t)ix->num_sms / B;
-        if (g->parts > 16) g->parts = 16;
+        const uint32_t fit = (uint32_t)ix->num_sms / B;
+        g->parts = fit >= 16 ? 16u : fit >= 8 ? 8u : fit >= 4 ? 4u : 2u;   // a power of two (pairwise merge)
     }
     g->cap = (k <= 256 || g->ring) ? 4096u : 8192u;            // the ring takes the shared memory of the larger buffer
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap, g->ring);
@@ -504,8 +504,8 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
     sp.out_ids = out_ids; sp.out_dists = out_dists; sp.out_counts = out_counts; sp.out_uniq = out_uniq;
     sp.parts = g.parts; sp.part_keys = (unsigned long long *)(ws + w.part_keys);
-    uint32_t merge_n2 = 32;
-    while (merge_n2 < g.parts * k) merge_n2 <<= 1;
+    uint32_t merge_k2 = 32;                                    // a part's keys padded to a power of two
+    while (merge_k2 < k) merge_k2 <<= 1;
     const int per_sm = dump ? 1 : scan_ctas_per_sm(ix, g.scan_smem);
 
     // With chunks > 1 the partition launches of all chunks go to the side stream at once: the partition kernel is
@@ -547,8 +547,8 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         if (timing) cudaEventRecord(ix->ev_scan[c][0], stream);
         cudaError_t e = launch_scan(ix, grid, g.scan_smem, stream, sp);
         if (e == cudaSuccess && g.parts > 1) {
-            merge_parts_kernel<<<qe - qb, kMergeThreads, (size_t)merge_n2 * 8, stream>>>(
-                sp.part_keys, uniq_counts, qb, g.parts, k, merge_n2, out_ids, out_dists, out_counts, out_uniq);
+            merge_parts_kernel<<<qe - qb, kMergeThreads, (size_t)g.parts * merge_k2 * 8, stream>>>(
+                sp.part_keys, uniq_counts, qb, g.parts, k, merge_k2, out_ids, out_dists, out_counts, out_uniq);
             ix->launches++;
             e = cudaGetLastError();
         }
@@ -801,8 +801,10 @@ extern "C" int fann_search_lists(fann_index *ix, const float *lut, uint32_t B, c
                                                          (unsigned long long *)offsets);
     lists_scan_kernel<<<1, 1024, 0, stream>>>((const unsigned long long *)offsets, B, offsets, hdr,
                                               (unsigned long long)max_total_cands);
-    lists_expand_kernel<<<B, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(ix->list_offsets, ix->list_ids, ix->n_lists,
-                                                                                probes, nprobe, offsets, ids, hdr);
+    uint32_t expand_ctas = 1;                                  // small batches: spread a query's lists over several CTAs
+    while (expand_ctas < 16 && 2 * expand_ctas * B <= (uint32_t)ix->num_sms && 8 * expand_ctas < nprobe) expand_ctas <<= 1;
+    lists_expand_kernel<<<B * expand_ctas, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(
+        ix->list_offsets, ix->list_ids, ix->n_lists, probes, nprobe, offsets, ids, hdr, expand_ctas);
     ix->launches += 3;
     CUDA_TRY(cudaGetLastError());
     // a batch larger than the workspace was sized for leaves cand_offsets[B] > max_total_cands: the path refuses it

@@ -85,18 +85,21 @@ __global__ void lists_scan_kernel(const unsigned long long *per_query, uint32_t 
 
 constexpr int kExpandThreads = 256;
 
-// One CTA per query: its probed lists' IDs concatenated in probe order at cand_ids + cand_offsets[b]
+// One CTA per query (or several, for small batches): its probed lists' IDs concatenated in probe order at cand_ids + cand_offsets[b]
 // (PAPER.md:L125 step (3)).  Dynamic shared memory: nprobe + 1 start positions.
 __global__ void __launch_bounds__(kExpandThreads) lists_expand_kernel(const long long *__restrict__ list_offsets,
                                                                       const uint32_t *__restrict__ list_ids, uint64_t n_lists,
                                                                       const uint32_t *__restrict__ probes, uint32_t nprobe,
                                                                       const long long *__restrict__ cand_offsets,
-                                                                      uint32_t *__restrict__ cand_ids, const ListsHeader *hdr)
+                                                                      uint32_t *__restrict__ cand_ids, const ListsHeader *hdr,
+                                                                      uint32_t ctas_per_query)
 {
     extern __shared__ uint32_t start[];                           // [nprobe + 1] positions inside the query's list
     __shared__ uint32_t carry;
     if (hdr->overflow) return;                                    // the workspace cannot hold the batch: write nothing
-    const uint32_t b = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // small batches: several CTAs per query share its lists (CTA `sub` copies lists sub * 8 + warp, + 8 * ctas, ...)
+    const uint32_t b = blockIdx.x / ctas_per_query, sub = blockIdx.x - b * ctas_per_query;
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t *pr = probes + (size_t)b * nprobe;
     if (tid == 0) carry = 0;
     __syncthreads();
@@ -125,7 +128,7 @@ __global__ void __launch_bounds__(kExpandThreads) lists_expand_kernel(const long
     if (tid == 0) start[nprobe] = carry;
     __syncthreads();
     uint32_t *out = cand_ids + cand_offsets[b];
-    for (uint32_t j = warp; j < nprobe; j += kExpandThreads / 32) {
+    for (uint32_t j = sub * (kExpandThreads / 32) + warp; j < nprobe; j += ctas_per_query * (kExpandThreads / 32)) {
         const uint32_t len = start[j + 1] - start[j];
         if (!len) continue;
         const uint32_t *src = list_ids + __ldg(list_offsets + __ldg(pr + j));
