@@ -166,14 +166,8 @@ def gather_ceiling(fann, ix, w, dev, nq_groups: int = 4):
     each sweeping one query's distinct list as the dedup kernel leaves it), with none of its arithmetic.  The
     distinct lists come from fann_dedup_only on the first queries of the timed batch.  Returns rows/s of the
     scan kernel's fill path (cp.async ring), of the sm_100 TMA gather4 flavour and of the same rows shuffled."""
-    import ctypes as C
     import torch
-    from paper_2409_16576_b200.build import build_probe
-    lib = C.CDLL(build_probe())
-    lib.fann_probe_gather.restype = C.c_int
-    lib.fann_probe_gather.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p,
-                                      C.c_uint32, C.c_uint32, C.c_void_p]
-    lib.fann_probe_last_error.restype = C.c_char_p
+    lib = _probe_lib()
     info = ix.info()
     sms, row_bytes, N = info["num_sms"], info["row_bytes"], info["N"]
     nq = min(w.cfg.B, nq_groups * sms) // sms * sms
@@ -223,6 +217,92 @@ def gather_ceiling(fann, ix, w, dev, nq_groups: int = 4):
     return {"rows": int(own.numel()), "queries": nq,
             "own_order_cp_async_ring": rate(own, 3), "own_order_tma_gather4": rate(own, 4),
             "shuffled_cp_async_ring": rate(rnd, 3)}
+
+
+def _probe_lib():
+    import ctypes as C
+    from paper_2409_16576_b200.build import build_probe
+    lib = C.CDLL(build_probe())
+    lib.fann_probe_gather.restype = C.c_int
+    lib.fann_probe_gather.argtypes = [C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p,
+                                      C.c_uint32, C.c_uint32, C.c_void_p]
+    lib.fann_probe_last_error.restype = C.c_char_p
+    return lib
+
+
+def probe_sweep(args, cfg):
+    """--probe-sweep: MEASUREMENT ONLY (include/fann_probe.h).  What bounds a gather of code rows on this part, on a
+    synthetic code array of the workload's size (contents are irrelevant to a read): every issue flavour of the probe
+    x {random, ascending inside each CTA's list} x {1, 2 CTAs per SM}, and the address-translation test -- random rows
+    confined to K random 2 MB pages of the array.  One JSON line; profiles/r2_gather_ceiling.md is written from it."""
+    import torch
+    lib = _probe_lib()
+    dev = "cuda:0"
+    torch.cuda.set_device(0)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    N, M = cfg.N, cfg.M
+    row_bytes = 16 if M <= 16 else (32 if M <= 32 else 64)
+    codes = torch.empty(N * row_bytes, dtype=torch.uint8, device=dev)
+    codes.view(torch.int64)[:] = 0x0102030405060708
+    sink = torch.zeros(4, dtype=torch.int32, device=dev)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(1)
+    stream = torch.cuda.current_stream().cuda_stream
+    rps = 2048 // row_bytes
+    unit = 16 * rps
+    U = max(unit, int(0.58 * cfg.nprobe * cfg.mean_list) // unit * unit)        # rows of one query's distinct list
+    groups = max(1, min(8, 40_000_000 // (sms * U)))
+
+    def lists(order):
+        out = []
+        for _ in range(groups):
+            ids = torch.randint(0, N, (sms, U), device=dev, generator=gen, dtype=torch.int64)
+            if order == "ascending":
+                ids = ids.sort(dim=1).values
+            out.append(ids.view(sms, U // unit, 16, rps).permute(1, 0, 2, 3).reshape(-1))
+        return torch.cat(out).to(torch.int32).contiguous()
+
+    def rate(ids, flavor, cps):
+        best = None
+        for it in range(4):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            rc = lib.fann_probe_gather(codes.data_ptr(), row_bytes, N, ids.data_ptr(), ids.numel(), sink.data_ptr(),
+                                       flavor, cps, stream)
+            b.record()
+            b.synchronize()
+            if rc != 0:
+                return None
+            if it:
+                t = a.elapsed_time(b)
+                best = t if best is None else min(best, t)
+        return round(ids.numel() / best / 1e6, 2)                               # G rows/s
+
+    names = {0: "ldg16", 1: "ldg16_l2_64", 2: "ldg32", 3: "cp_async_ring", 4: "tma_gather4"}
+    flavors = [f for f in (0, 1, 2, 3, 4) if not (f == 2 and row_bytes < 32)]
+    sweep = []
+    for order in ("random", "ascending"):
+        ids = lists(order)
+        for f in flavors:
+            for cps in (1, 2):
+                sweep.append({"order": order, "flavor": names[f], "ctas_per_sm": cps, "rows": int(ids.numel()),
+                              "G_rows_per_s": rate(ids, f, cps)})
+    # address translation: random rows confined to K random 2 MB pages of the array
+    page_rows = (2 << 20) // row_bytes
+    npages = N // page_rows
+    n = groups * sms * U
+    pages_test = []
+    for K in (256, 1024, 4096, 16384, npages):
+        if K > npages:
+            continue
+        pg = torch.randperm(npages, device=dev, generator=gen)[:K]
+        ids = (pg[torch.randint(0, K, (n,), device=dev, generator=gen)] * page_rows +
+               torch.randint(0, page_rows, (n,), device=dev, generator=gen)).to(torch.int32)
+        pages_test.append({"pages_2MB": int(K), "footprint_GB": round(K * (2 << 20) / 1e9, 2),
+                           "G_rows_per_s": rate(ids, 3, 1)})
+    print(json.dumps({"probe_sweep": {"workload": cfg.name, "N": N, "row_bytes": row_bytes, "array_GB": round(N * row_bytes / 1e9, 1),
+                                      "rows_per_cta_list": U, "sms": sms, "order_x_flavor": sweep,
+                                      "random_rows_in_K_pages": pages_test}}))
 
 
 def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=False, sample_clocks=False):
@@ -401,6 +481,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-ceiling", action="store_true", help="skip the gather-ceiling probe leg")
     ap.add_argument("--no-configs", action="store_true", help="skip the block with the other large workloads")
+    ap.add_argument("--probe-sweep", action="store_true",
+                    help="measurement only: the row-gather ceiling sweep on a synthetic array of the workload's size")
     ap.add_argument("--id-map", default=None, choices=["feistel", "lattice"],
                     help="vector -> ID map of the generator (default: the config's, 'feistel')")
     args = ap.parse_args()
@@ -419,6 +501,10 @@ def main():
 
     if args.impl == "reference":
         return reference_arm(args, cfg, rank, world)
+    if args.probe_sweep:
+        if rank == 0:
+            probe_sweep(args, cfg)
+        return
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback"
     torch.cuda.set_device(local_rank)

@@ -1032,9 +1032,11 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             U = (c1 < U ? c1 : U) - (c0 < U ? c0 : U);
         }
 
-        {   // stage the lookup table c-major; each warp writes 32 different banks per store
+        // stage the lookup table c-major; each warp writes 32 different banks per store
+        auto stage_lut = [&]() {
             constexpr uint32_t ncols = G == 4 ? 64 : 32;
             const float4 *g4 = reinterpret_cast<const float4 *>(p.lut + (size_t)b * p.M * 256);
+#pragma unroll 4
             for (uint32_t i = tid; i < ncols * 64; i += kScanThreads) {
                 const uint32_t col = i % ncols, c4 = i / ncols;
                 const uint32_t m = m_of_col<G>(col);
@@ -1044,8 +1046,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                 d[0] = v.x; d[64] = v.y; d[128] = v.z; d[192] = v.w;
             }
             if (tid == 0) { misc[0] = 0; misc[9] = 0; *tau_p = kKeyMax; }
-        }
-        __syncthreads();
+        };
 
         if constexpr (D > 0) {
             const uint32_t ring = (uint32_t)__cvta_generic_to_shared(lutb + 65536) + warp * (D * kRingStageBytes);
@@ -1080,9 +1081,12 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                 }
                 cp_async_commit();                             // one group per stage, empty past the end
             };
+            // the first row copies go out before the table is staged: they need the IDs only, and fly meanwhile
             load_ids(0);
 #pragma unroll
             for (int d = 0; d < D - 1; ++d) issue(d);
+            stage_lut();
+            __syncthreads();
             uint32_t st = 0;
             for (;;) {
                 while (st < n_st && !vm[9]) {
@@ -1124,6 +1128,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             }
             cp_async_wait<0>();
         } else {
+            stage_lut();
+            __syncthreads();
             const uint32_t per_iter = kScanWarps * 32 * NB;
             const uint32_t n_iter = (U + per_iter - 1) / per_iter;
             // Warps run free: no barrier per iteration.  The warp whose append takes the buffer past its limit
