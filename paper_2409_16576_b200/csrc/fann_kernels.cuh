@@ -602,7 +602,10 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
             uint32_t off = kNoSlot;
             if (BS == 4) {
                 const uint4 v = lds_u128(a);
-                const uint32_t hv = lds_u32(a + home);
+                // the home slot's value out of the four just read (a second, 4-byte load costs more: the kernel
+                // is bound by shared-memory wavefronts -- random 16-byte reads conflict 2.7x -- as much as by issue)
+                const uint32_t hlo = (home & 4u) ? v.y : v.x, hhi = (home & 4u) ? v.w : v.z;
+                const uint32_t hv = (home & 8u) ? hhi : hlo;
                 found = v.x == x || v.y == x || v.z == x || v.w == x;
                 off = v.w == kEmpty ? 12u : off;
                 off = v.z == kEmpty ? 8u : off;
