@@ -250,6 +250,31 @@ int fann_search_lists_host(fann_index *ix, const float *queries_h, uint32_t B,
                            void *device_scratch, size_t scratch_bytes, void *stream);
 
 /*
+ * EXPERIMENT -- a list-major copy of the codes, streamed instead of gathered.  NOT the paper's
+ * layout: the paper keeps one code per vector, indexed by vector-ID, and the
+ * posting lists hold vector-IDs only (L150); this keeps, in addition, the codes in posting-list
+ * order, replicas included (list_entries x row_bytes of HBM: 64 GB more at 10^9 entries of
+ * 64-byte codes), so that step (6) reads each probed list as one contiguous run.  Every
+ * candidate is scored, repeats included; the repeats (a vector in several probed lists has the
+ * same distance and ID each time) are removed exactly where the top-k buffer is pruned, so
+ * steps (5)-(7) need no dedup pass.  Results are the bytes of fann_search_lists.
+ *
+ * fann_build_list_codes builds the copy from the loaded codes and posting lists (enqueues on
+ * `stream`; loading other lists discards it).  fann_search_lists_stream is fann_search_lists
+ * on it, without out_uniq (the distinct candidates are never counted).  Its workspace holds
+ * the batch's (row, vector-ID) pairs only (8 bytes per candidate).  fann_search_lists_stream_status
+ * synchronises `stream` and returns FANN_OK or FANN_EWORKSPACE (max_total_cands too small;
+ * *total_cands, may be NULL, receives the count that was needed).
+ */
+int fann_build_list_codes(fann_index *ix, void *stream);
+size_t fann_search_lists_stream_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t max_total_cands);
+int fann_search_lists_stream(fann_index *ix, const float *lut, uint32_t B,
+                             const uint32_t *probes, uint32_t nprobe, uint64_t max_total_cands, uint32_t k,
+                             uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
+                             void *workspace, size_t workspace_bytes, void *stream);
+int fann_search_lists_stream_status(fann_index *ix, const void *workspace, uint64_t *total_cands, void *stream);
+
+/*
  * NEXT-3 -- low-latency small-batch serving, PAPER.md:L204-L208 (section 5): "each CPU thread
  * handles an individual query" and a "contention-free GPU memory manager": the HBM left after
  * the codes is cut into fixed blocks, a block is handed to a query and recycled.

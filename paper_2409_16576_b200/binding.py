@@ -79,6 +79,10 @@ def load_library():
         "fann_search_lists_status": (i, [p, p, u32, u64, u32, C.POINTER(u64), p]),
         "fann_search_lists_host_scratch_bytes": (sz, [p, u32, u32, u32, u64, u32]),
         "fann_search_lists_host": (i, [p, p, u32, p, u32, p, u32, u64, u32, p, p, p, p, sz, p]),
+        "fann_build_list_codes": (i, [p, p]),
+        "fann_search_lists_stream_workspace_bytes": (sz, [p, u32, u64]),
+        "fann_search_lists_stream": (i, [p, p, u32, p, u32, u64, u32, p, p, p, p, sz, p]),
+        "fann_search_lists_stream_status": (i, [p, p, C.POINTER(u64), p]),
         "fann_pool_create": (i, [p, u32, u32, u64, u32, u32, u32, C.POINTER(p)]),
         "fann_pool_destroy": (None, [p]),
         "fann_pool_stats": (i, [p, C.POINTER(_PoolInfo)]),
@@ -228,6 +232,35 @@ def fann_search_lists_host(ix, queries_h, B, codebooks_d, dsub, probes_h, nprobe
     _check(load_library().fann_search_lists_host(ix, _addr(queries_h), B, _addr(codebooks_d), dsub, _addr(probes_h),
                                                  nprobe, max_total_cands, k, _addr(out_ids_h), _addr(out_dists_h),
                                                  _addr(out_counts_h), _addr(device_scratch), scratch_bytes, stream))
+
+
+def fann_build_list_codes(ix, stream=None) -> None:
+    _check(load_library().fann_build_list_codes(ix, stream))
+
+
+def fann_search_lists_stream_workspace_bytes(ix, B, max_total_cands) -> int:
+    n = load_library().fann_search_lists_stream_workspace_bytes(ix, B, max_total_cands)
+    if n == 0:
+        raise FannError(-1, fann_last_error())
+    return n
+
+
+def fann_search_lists_stream(ix, lut, B, probes, nprobe, max_total_cands, k, out_ids, out_dists, out_counts,
+                             workspace, workspace_bytes, stream=None) -> None:
+    _check(load_library().fann_search_lists_stream(ix, _addr(lut), B, _addr(probes), nprobe, max_total_cands, k,
+                                                   _addr(out_ids), _addr(out_dists), _addr(out_counts),
+                                                   _addr(workspace), workspace_bytes, stream))
+
+
+def fann_search_lists_stream_status(ix, workspace, stream=None) -> int:
+    """Raises on a bad status; returns the batch's candidate count."""
+    total = C.c_uint64(0)
+    rc = load_library().fann_search_lists_stream_status(ix, _addr(workspace), C.byref(total), stream)
+    if rc != FANN_OK:
+        err = FannError(rc, fann_last_error())
+        err.total_cands = int(total.value)
+        raise err
+    return int(total.value)
 
 
 def fann_pool_create(ix, n_blocks, max_B, max_cands, dsub, max_nprobe, k_max) -> int:

@@ -39,6 +39,7 @@ struct fann_index {
     uint64_t vec_N = 0;
     uint32_t vec_d = 0;
     int vec_elem = 0;
+    uint8_t *lm_codes = nullptr;           // list-major experiment: [list_entries][row_bytes], row e = code of list_ids[e]
     uint32_t *page_of = nullptr;           // [page_N]
     uint64_t page_N = 0, n_pages = 0;
     int num_sms = 0;
@@ -195,10 +196,10 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
 extern "C" const char *fann_last_error(void) { return g_err; }
 extern "C" const char *fann_version(void) { return "fann 0.3 sm_100a"; }
 
-template <int G, int NB, int D>
+template <int G, int NB, int D, bool LM = false>
 static cudaError_t set_scan_attr(int smem)
 {
-    return cudaFuncSetAttribute(scan_kernel<G, NB, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    return cudaFuncSetAttribute(scan_kernel<G, NB, D, LM>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
 extern "C" int fann_create(fann_index **out, int device)
@@ -231,6 +232,9 @@ extern "C" int fann_create(fann_index **out, int device)
     CUDA_TRY((set_scan_attr<1, 4, 3>(ring_max)));
     CUDA_TRY((set_scan_attr<2, 4, 3>(ring_max)));
     CUDA_TRY((set_scan_attr<4, 2, 3>(ring_max)));
+    CUDA_TRY((set_scan_attr<1, 4, 3, true>(ring_max)));
+    CUDA_TRY((set_scan_attr<2, 4, 3, true>(ring_max)));
+    CUDA_TRY((set_scan_attr<4, 2, 3, true>(ring_max)));
     CUDA_TRY(cudaFuncSetAttribute(merge_parts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 16384 * 8));
     int per_sm = 0;
     CUDA_TRY(cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device));
@@ -261,6 +265,7 @@ extern "C" void fann_destroy(fann_index *ix)
     if (ix->list_ids) cudaFree(ix->list_ids);
     if (ix->vectors) cudaFree(ix->vectors);
     if (ix->page_of) cudaFree(ix->page_of);
+    if (ix->lm_codes) cudaFree(ix->lm_codes);
     for (CallCtx *c : ix->ctx_pool) destroy_ctx(c);
     for (auto &e : ix->ev_lut) if (e) cudaEventDestroy(e);
     for (auto &e : ix->ev_plan) if (e) cudaEventDestroy(e);
@@ -403,6 +408,14 @@ extern "C" size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_
 
 static cudaError_t launch_scan(const fann_index *ix, int grid, size_t smem, cudaStream_t stream, const ScanParams &p)
 {
+    if (p.key_src) {                                           // list-major experiment (ring only)
+        switch (ix->row_bytes) {
+        case 16: scan_kernel<1, 4, 3, true><<<grid, kScanThreads, smem, stream>>>(p); break;
+        case 32: scan_kernel<2, 4, 3, true><<<grid, kScanThreads, smem, stream>>>(p); break;
+        default: scan_kernel<4, 2, 3, true><<<grid, kScanThreads, smem, stream>>>(p); break;
+        }
+        return cudaGetLastError();
+    }
     if (ix->scan_ring) switch (ix->row_bytes) {
     case 16: scan_kernel<1, 4, 3><<<grid, kScanThreads, smem, stream>>>(p); break;
     case 32: scan_kernel<2, 4, 3><<<grid, kScanThreads, smem, stream>>>(p); break;
@@ -504,6 +517,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
     sp.out_ids = out_ids; sp.out_dists = out_dists; sp.out_counts = out_counts; sp.out_uniq = out_uniq;
     sp.parts = g.parts; sp.part_keys = (unsigned long long *)(ws + w.part_keys);
+    sp.key_src = nullptr; sp.id_limit = 0xFFFFFFFFu;
     uint32_t merge_k2 = 32;                                    // a part's keys padded to a power of two
     while (merge_k2 < k) merge_k2 <<= 1;
     const int per_sm = dump ? 1 : scan_ctas_per_sm(ix, g.scan_smem);
@@ -726,6 +740,7 @@ extern "C" int fann_load_lists(fann_index *ix, const int64_t *list_offsets, cons
     cudaStream_t stream = (cudaStream_t)stream_;
     if (ix->list_offsets) { cudaFree(ix->list_offsets); ix->list_offsets = nullptr; }
     if (ix->list_ids) { cudaFree(ix->list_ids); ix->list_ids = nullptr; }
+    if (ix->lm_codes) { cudaFree(ix->lm_codes); ix->lm_codes = nullptr; }      // built from the old lists
     ix->n_lists = 0; ix->list_entries = 0;
     cudaError_t e = cudaMalloc(&ix->list_offsets, (n_lists + 1) * 8);
     if (e == cudaSuccess) e = cudaMalloc(&ix->list_ids, (n_entries ? n_entries : 1) * 4);
@@ -792,7 +807,7 @@ static int search_lists_impl(fann_index *ix, const float *lut, uint32_t B, const
     uint32_t expand_ctas = 1;                                  // small batches: spread a query's lists over several CTAs
     while (expand_ctas < 16 && 2 * expand_ctas * B <= (uint32_t)ix->num_sms && 8 * expand_ctas < nprobe) expand_ctas <<= 1;
     lists_expand_kernel<<<B * expand_ctas, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(
-        ix->list_offsets, ix->list_ids, ix->n_lists, probes, nprobe, offsets, ids, hdr, expand_ctas);
+        ix->list_offsets, ix->list_ids, ix->n_lists, probes, nprobe, offsets, ids, hdr, expand_ctas, 0u);
     ix->launches += 3;
     CUDA_TRY(cudaGetLastError());
     // a batch larger than the workspace was sized for leaves cand_offsets[B] > max_total_cands: the path refuses it
@@ -929,6 +944,124 @@ extern "C" int fann_search_lists_host(fann_index *ix, const float *queries_h, ui
         CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_fork, 0));     // `stream` ends after the last copy
     }
     return fann_search_lists_status(ix, s + h.ws, B, max_total_cands, k, nullptr, stream);   // synchronises
+}
+
+// ---------------------------------------------------------------- EXPERIMENT: list-major code copy, streamed
+
+// Not the paper's layout (its codes are indexed by vector-ID, L152, and the lists hold IDs only, L150): a second copy
+// of the codes in posting-list order, replicas included, so that step (6) reads a probed list as one contiguous run
+// instead of gathering rows.  Every candidate is scored, repeats included; they are removed where the top-k buffer is
+// pruned (a vector in several probed lists has the same key each time).  See DESIGN.md 6.7.
+extern "C" int fann_build_list_codes(fann_index *ix, void *stream_)
+{
+    if (!ix) return fail(FANN_EINVAL, "fann_build_list_codes: NULL index");
+    if (!ix->codes || !ix->list_offsets) return fail(FANN_EINVAL, "fann_build_list_codes: load codes and posting lists first");
+    if (ix->list_entries >= 0xFFFFFFFFull) return fail(FANN_EUNSUPPORTED, "fann_build_list_codes: more than 2^32-2 list entries");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (ix->lm_codes) { cudaFree(ix->lm_codes); ix->lm_codes = nullptr; }
+    const size_t bytes = (size_t)(ix->list_entries ? ix->list_entries : 1) * ix->row_bytes;
+    cudaError_t e = cudaMalloc(&ix->lm_codes, bytes);
+    if (e != cudaSuccess) { ix->lm_codes = nullptr; return fail(FANN_ENOMEM, "fann_build_list_codes: cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); }
+    const uint32_t chunks = ix->row_bytes >> 4;
+    const uint64_t per_launch = 1ull << 26;
+    for (uint64_t e0 = 0; e0 < ix->list_entries; e0 += per_launch) {
+        const uint64_t n = ix->list_entries - e0 < per_launch ? ix->list_entries - e0 : per_launch;
+        list_codes_kernel<<<(unsigned)((n * chunks + 255) / 256), 256, 0, stream>>>(ix->codes, ix->N, ix->row_bytes, ix->list_ids,
+                                                                                  e0, n, ix->lm_codes);
+        ix->launches++;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return FANN_OK;
+}
+
+struct StreamLayout { size_t hdr, counter, counts, offsets, rows, total; };
+
+static void stream_layout(uint32_t B, uint64_t cap, StreamLayout *l)
+{
+    size_t o = 0;
+    l->hdr = o;     o = align_up(o + sizeof(ListsHeader), 256);
+    l->counter = o; o = align_up(o + 256, 256);
+    l->counts = o;  o = align_up(o + (size_t)B * 4, 256);
+    l->offsets = o; o = align_up(o + ((size_t)B + 1) * 8, 256);
+    l->rows = o;    o = align_up(o + (size_t)cap * 8 + 16, 256);      // (row, vector-ID) per candidate
+    l->total = o;
+}
+
+extern "C" size_t fann_search_lists_stream_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t max_total_cands)
+{
+    if (!ix || B == 0) { fail(FANN_EINVAL, "fann_search_lists_stream_workspace_bytes: bad argument"); return 0; }
+    StreamLayout l;
+    stream_layout(B, max_total_cands, &l);
+    return l.total;
+}
+
+__global__ void stream_counts_kernel(const long long *__restrict__ offsets, uint32_t B, uint32_t *__restrict__ counts,
+                                     uint32_t *counter, const fann::ListsHeader *hdr)
+{
+    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b == 0) *counter = 0;
+    if (b < B) counts[b] = hdr->overflow ? 0u : (uint32_t)(offsets[b + 1] - offsets[b]);
+}
+
+extern "C" int fann_search_lists_stream(fann_index *ix, const float *lut, uint32_t B, const uint32_t *probes, uint32_t nprobe,
+                                        uint64_t max_total_cands, uint32_t k, uint32_t *out_ids, float *out_dists,
+                                        uint32_t *out_counts, void *workspace, size_t workspace_bytes, void *stream_)
+{
+    if (!ix || !lut || !probes || !out_ids || !out_dists) return fail(FANN_EINVAL, "fann_search_lists_stream: NULL argument");
+    if (!ix->lm_codes) return fail(FANN_EINVAL, "fann_search_lists_stream: build the list-major copy first (fann_build_list_codes)");
+    if (B == 0 || nprobe == 0) return fail(FANN_EINVAL, "fann_search_lists_stream: B or nprobe is 0");
+    if (nprobe > FANN_MAX_NPROBE) return fail(FANN_EUNSUPPORTED, "fann_search_lists_stream: nprobe=%u > %u", nprobe, FANN_MAX_NPROBE);
+    if (k == 0 || k > FANN_MAX_K) return fail(FANN_EUNSUPPORTED, "fann_search_lists_stream: k=%u not in 1..%u", k, FANN_MAX_K);
+    if (!ix->scan_ring) return fail(FANN_EUNSUPPORTED, "fann_search_lists_stream: needs the ring scan (FANN_SCAN_RING=0 is set)");
+    if (((uintptr_t)probes & 3) != 0 || ((uintptr_t)lut & 15) != 0) return fail(FANN_EINVAL, "fann_search_lists_stream: misaligned probes or lut");
+    StreamLayout l;
+    stream_layout(B, max_total_cands, &l);
+    if (!workspace || ((uintptr_t)workspace & 255) != 0) return fail(FANN_EWORKSPACE, "workspace is NULL or not 256-byte aligned");
+    if (workspace_bytes < l.total) return fail(FANN_EWORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, l.total);
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    char *ws = (char *)workspace;
+    ListsHeader *hdr = (ListsHeader *)(ws + l.hdr);
+    long long *offsets = (long long *)(ws + l.offsets);
+    uint32_t *rows = (uint32_t *)(ws + l.rows), *counts = (uint32_t *)(ws + l.counts), *counter = (uint32_t *)(ws + l.counter);
+    lists_count_kernel<<<(B + 7) / 8, 256, 0, stream>>>(ix->list_offsets, ix->n_lists, probes, B, nprobe,
+                                                         (unsigned long long *)offsets);
+    lists_scan_kernel<<<1, 1024, 0, stream>>>((const unsigned long long *)offsets, B, offsets, hdr,
+                                              (unsigned long long)max_total_cands, 0u);
+    lists_expand_kernel<<<B, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(
+        ix->list_offsets, ix->list_ids, ix->n_lists, probes, nprobe, offsets, rows, hdr, 1u, 1u);
+    stream_counts_kernel<<<(B + 255) / 256, 256, 0, stream>>>(offsets, B, counts, counter, hdr);
+    ix->launches += 4;
+    CUDA_TRY(cudaGetLastError());
+    Geom g;
+    geometry(ix, k, B, max_total_cands, &g, 0, false);
+    ScanParams sp;
+    sp.codes = ix->lm_codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = offsets; sp.uniq_ids = rows; sp.uniq_counts = counts;
+    sp.k = k; sp.cap = g.cap; sp.q_begin = 0; sp.q_end = B; sp.counter = counter;
+    sp.out_ids = out_ids; sp.out_dists = out_dists; sp.out_counts = out_counts; sp.out_uniq = nullptr;
+    sp.parts = 1; sp.part_keys = nullptr; sp.key_src = rows; sp.id_limit = (uint32_t)ix->N;
+    int grid = ix->num_sms * scan_ctas_per_sm(ix, g.scan_smem);
+    if ((uint32_t)grid > B) grid = (int)B;
+    cudaError_t e = launch_scan(ix, grid, g.scan_smem, stream, sp);
+    ix->launches++;
+    if (e != cudaSuccess) return fail(FANN_ECUDA, "scan kernel launch: %s", cudaGetErrorString(e));
+    return FANN_OK;
+}
+
+extern "C" int fann_search_lists_stream_status(fann_index *ix, const void *workspace, uint64_t *total_cands, void *stream_)
+{
+    if (!ix || !workspace) return fail(FANN_EINVAL, "fann_search_lists_stream_status: NULL argument");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    ListsHeader h;
+    CUDA_TRY(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    if (total_cands) *total_cands = h.total;
+    if (h.overflow)
+        return fail(FANN_EWORKSPACE, "the probed lists hold %llu candidate IDs, the workspace was sized for %llu (max_total_cands)",
+                    h.total, h.capacity);
+    return FANN_OK;
 }
 
 // ---------------------------------------------------------------- NEXT-3: low-latency small-batch serving

@@ -404,37 +404,46 @@ __global__ void __launch_bounds__(kPartThreads) partition_kernel(const PartParam
         if (v < nvec) return load_ids4(ids, 4ll * v - shift, C);
         return make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
     };
+    const uint32_t N32 = (uint32_t)p.N;                        // N < 2^32 - 1 (fann_load_codes)
     for (;;) {
         const uint32_t MS = hashed ? 0u : ordered_class_mul(p.N, S);
         if (tid < kMaxPartBuckets) scnt[tid] = 0;
         __syncthreads();
-        bool overflow = false;
+        uint32_t overflow = 0;
+        // One ID: its class; lanes of the same class found by one MATCH instead of a ballot per class; the lowest
+        // lane of each class reserves the class's output range for all of them.  (Issuing the four matches of a
+        // vector before using any result was measured slower: 2.68 against 2.51 ms.)
+        auto place = [&](uint32_t x, uint32_t cls) {
+            const bool valid = x < N32;                        // also drops kIdNone
+            if (!valid) cls = 0xFFu;
+            const uint32_t own = __match_any_sync(0xffffffffu, cls);
+            const uint32_t leader = __ffs(own) - 1;
+            uint32_t base = 0;
+            if (valid && lane == leader) base = atoms_add(scnt_addr + (cls << 2), (uint32_t)__popc(own));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            const uint32_t pos = base + __popc(own & lt_mask);
+            if (valid) {
+                if (pos < capb) out[cls * capb + pos] = x;     // cls * capb + pos < 2 C < 2^32
+                else overflow = 1;
+            }
+        };
         uint4 nxt = load_vec(tid);
-        for (uint32_t vb = 0; vb < nvec; vb += kPartThreads) { // uniform trip count: ballots below need whole warps
-            const uint4 q4 = nxt;
-            nxt = load_vec(vb + kPartThreads + tid);           // one iteration ahead
-            const uint32_t x[4] = {q4.x, q4.y, q4.z, q4.w};
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const bool valid = (uint64_t)x[e] < p.N;       // also drops kIdNone
-                uint32_t cls = hashed ? __umulhi(hash_round1(x[e]), S) : __umulhi(x[e], MS);
-                if (!valid) cls = 0xFFu;
-                // lanes of the same class: one MATCH instead of a ballot per class; the lowest lane of each
-                // class reserves the class's output range for all of them.  (Issuing the four matches of a
-                // vector before using any result was measured slower: 2.68 against 2.51 ms.)
-                const uint32_t own = __match_any_sync(0xffffffffu, cls);
-                const uint32_t leader = __ffs(own) - 1;
-                uint32_t base = 0;
-                if (valid && lane == leader) base = atoms_add(scnt_addr + (cls << 2), (uint32_t)__popc(own));
-                base = __shfl_sync(0xffffffffu, base, leader);
-                const uint32_t pos = base + __popc(own & lt_mask);
-                if (valid) {
-                    if (pos < capb) out[(size_t)cls * capb + pos] = x[e];
-                    else overflow = true;
-                }
+        if (!hashed) {
+            for (uint32_t vb = 0; vb < nvec; vb += kPartThreads) { // uniform trip count: the matches need whole warps
+                const uint4 q4 = nxt;
+                nxt = load_vec(vb + kPartThreads + tid);           // one iteration ahead
+                place(q4.x, __umulhi(q4.x, MS)); place(q4.y, __umulhi(q4.y, MS));
+                place(q4.z, __umulhi(q4.z, MS)); place(q4.w, __umulhi(q4.w, MS));
+            }
+        } else {
+            for (uint32_t vb = 0; vb < nvec; vb += kPartThreads) {
+                const uint4 q4 = nxt;
+                nxt = load_vec(vb + kPartThreads + tid);
+                place(q4.x, __umulhi(hash_round1(q4.x), S)); place(q4.y, __umulhi(hash_round1(q4.y), S));
+                place(q4.z, __umulhi(hash_round1(q4.z), S)); place(q4.w, __umulhi(hash_round1(q4.w), S));
             }
         }
-        bool bad = __syncthreads_or(overflow);                  // also: every scnt[] update is visible
+        bool bad = __syncthreads_or(overflow != 0);             // also: every scnt[] update is visible
         if (!hashed) {
             // exact class counts: an ID-range class that would overfill a dedup table if none of its IDs repeats
             const bool big = tid < S && scnt[tid] > p.class_max;
@@ -467,8 +476,11 @@ __device__ __forceinline__ uint4 load_ids4(const uint32_t *ids, long long e0, ui
 constexpr int kDedupIdsPerThread = 8;                // fresh IDs a thread holds per batch (two 16-byte loads)
 // bookkeeping (256 bytes, of which bytes 64..79 are a bucket that stays empty) + two retry queues of `threads`
 // (id, bucket address) pairs precede the table
-constexpr int kDedupBucketSlots = 4;                 // slots per bucket (2: one 8-byte look, 4: one 16-byte look)
-constexpr int kDedupQueuePer8 = kDedupBucketSlots == 2 ? 2 : 1;   // queued entries a thread takes up per batch, per 8 fresh IDs
+#ifndef FANN_DEDUP_BS
+#define FANN_DEDUP_BS 4
+#endif
+constexpr int kDedupBucketSlots = FANN_DEDUP_BS;                 // slots per bucket (2: one 8-byte look, 4: one 16-byte look)
+constexpr int kDedupQueuePer8 = kDedupBucketSlots == 1 ? 3 : kDedupBucketSlots == 2 ? 2 : 1;   // queued entries a thread takes up per batch, per 8 fresh IDs
 // `shape` = threads x fresh IDs per thread / 8: 1024 (one CTA per SM) or 512 (two CTAs per SM)
 __host__ __device__ constexpr uint32_t dedup_table_off(uint32_t shape) { return 256 + 2 * kDedupQueuePer8 * shape * 8; }
 
@@ -494,7 +506,7 @@ __host__ __device__ constexpr uint32_t dedup_table_off(uint32_t shape) { return 
 template <int T, int R>
 __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const DedupParams p)
 {
-    constexpr int BS = kDedupBucketSlots, BSH = BS == 2 ? 3 : 4;   // slots per bucket, log2 of its bytes
+    constexpr int BS = kDedupBucketSlots, BSH = BS == 1 ? 2 : BS == 2 ? 3 : 4;   // slots per bucket, log2 of its bytes
     constexpr int NV = R / 4, NQ = kDedupQueuePer8 * R / 8, NE = R + NQ;   // per thread and batch: NV vectors = R fresh IDs + NQ from the queue
     constexpr uint32_t QCAP = NQ * T;                          // entries one retry queue holds
     constexpr uint32_t kNoSlot = 4 * BS;                       // "no empty slot in this bucket" as a byte offset
@@ -612,12 +624,16 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
                 off = v.y == kEmpty ? 4u : off;
                 off = v.x == kEmpty ? 0u : off;
                 off = hv == kEmpty ? home : off;
-            } else {
+            } else if (BS == 2) {
                 const uint2 v = lds_u64(a);
                 found = v.x == x || v.y == x;
                 const uint32_t hv = home ? v.y : v.x, ov = home ? v.x : v.y;
                 off = ov == kEmpty ? home ^ 4u : off;
                 off = hv == kEmpty ? home : off;
+            } else {
+                const uint32_t v = lds_u32(a);
+                found = v == x;
+                off = v == kEmpty ? 0u : off;
             }
             if (found) x = kIdNone;
             return (found || off == kNoSlot) ? none_addr : a + off;
@@ -854,6 +870,11 @@ struct ScanParams {
     uint32_t *out_uniq;                              // [B] or NULL
     uint32_t parts;                                  // CTAs per query: > 1 splits a query's distinct list (small batches)
     unsigned long long *part_keys;                   // [B][parts][k] partial top-k keys, merged by merge_parts_kernel
+    // List-major experiment (fann_search_lists_stream): `codes` is the list-major copy, key_src holds (row of that
+    // copy, vector-ID) pairs WITH repeats, query b's at cand_offsets[b] (uniq_counts[b] = C_b); an ID >= id_limit is
+    // skipped, and the repeats are removed where the top-k buffer is pruned.  key_src == NULL otherwise.
+    const uint32_t *key_src;
+    uint32_t id_limit;                               // 0xFFFFFFFF (kIdNone only) on the ordinary path
 };
 
 // Column of sub-space m in the c-major shared-memory table.  G = 16-byte chunks (= lanes) per row.
@@ -949,6 +970,75 @@ __device__ __forceinline__ void prune(unsigned long long *buf, uint32_t *misc, u
     __syncthreads();
 }
 
+// List-major experiment: the buffer may hold a vector several times (once per probed list it sits in) -- with the
+// same distance on integer data, with distances a rounding apart on real-valued data (a row's summation order
+// depends on the lane that scores it).  Exact prune: sort by (id, dist), keep the first entry of every id, sort the
+// survivors by (dist, id), keep the k smallest; tau = the k-th + 1 once k distinct vectors exist.  On return
+// buf[0 .. *cnt) is ascending and holds every id once.
+__device__ __forceinline__ void prune_exact(unsigned long long *buf, uint32_t *misc, uint32_t *scratch, uint32_t k, uint32_t cap)
+{
+    volatile uint32_t *vm = misc;
+    unsigned long long *tau_p = reinterpret_cast<unsigned long long *>(misc + 4);
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t n = vm[0] < cap ? vm[0] : cap;
+    uint32_t P = 32;
+    while (P < n) P <<= 1;
+    for (uint32_t i = tid; i < P; i += kScanThreads) {         // (dist, id) -> (id, dist)
+        const unsigned long long x = i < n ? buf[i] : kKeyMax;
+        buf[i] = (x << 32) | (x >> 32);
+    }
+    __syncthreads();
+    bitonic_sort_smem(buf, P, 2);
+    constexpr int KPT = 8192 / kScanThreads;                   // keys per thread, consecutive (cap <= 8192)
+    unsigned long long key[KPT];
+    unsigned long long prev = (tid && tid * KPT - 1 < P) ? buf[tid * KPT - 1] : kKeyMax;
+    uint32_t c = 0, flags = 0;
+#pragma unroll
+    for (int j = 0; j < KPT; ++j) {
+        const uint32_t i = tid * KPT + j;
+        key[j] = i < P ? buf[i] : kKeyMax;
+        const bool first = key[j] != kKeyMax && (i == 0 || (uint32_t)(key[j] >> 32) != (uint32_t)(prev >> 32));
+        prev = key[j];
+        if (first) { flags |= 1u << j; ++c; }
+    }
+    uint32_t incl = c;                                         // block exclusive scan of c
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += u;
+    }
+    if (lane == 31) scratch[warp] = incl;
+    __syncthreads();                                           // also: every key is in registers, buf may be overwritten
+    if (warp == 0) {
+        const uint32_t wv = lane < kScanWarps ? scratch[lane] : 0u;
+        uint32_t wi = wv;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, wi, o);
+            if (lane >= o) wi += u;
+        }
+        if (lane < kScanWarps) scratch[lane] = wi - wv;
+        if (lane == kScanWarps - 1) scratch[kScanWarps] = wi;   // distinct ids in all
+    }
+    __syncthreads();
+    uint32_t pos = scratch[warp] + incl - c;
+#pragma unroll
+    for (int j = 0; j < KPT; ++j)
+        if (flags >> j & 1u) buf[pos++] = (key[j] << 32) | (key[j] >> 32);   // back to (dist, id)
+    const uint32_t d = scratch[kScanWarps];
+    uint32_t P2 = 32;
+    while (P2 < d) P2 <<= 1;
+    __syncthreads();
+    for (uint32_t i = d + tid; i < P2; i += kScanThreads) buf[i] = kKeyMax;
+    __syncthreads();
+    bitonic_sort_smem(buf, P2, 2);
+    if (tid == 0) {
+        if (d >= k) { misc[0] = k; *tau_p = buf[k - 1] + 1; }
+        else misc[0] = d;
+    }
+    __syncthreads();
+}
+
 // 16 table lookups for the 16 code bytes a lane holds (Eq. 1).  The byte address of
 // each lookup is built by one PRMT: byte 0 = this lane's column offset, byte 1 = the code.
 template <int G>
@@ -977,7 +1067,9 @@ __device__ __forceinline__ float adc16(const uint4 r, const unsigned char *lutb,
 // D = 0: code rows go through registers (NB row groups in flight per lane).  D >= 2: every warp keeps a
 // private ring of D stages in shared memory and fills it D - 1 stages ahead with 16-byte asynchronous
 // copies, so row reads stay in flight while the warp computes.
-template <int G, int NB, int D>
+// LM (list-major experiment): rows are numbered in the list-major copy, their vector-IDs come from p.key_src,
+// repeats are removed by prune_exact.  The ordinary path is LM = false and carries none of it.
+template <int G, int NB, int D, bool LM = false>
 __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 {
     constexpr int ROWB = 16 * G;
@@ -1055,13 +1147,20 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
             const uint32_t ring = (uint32_t)__cvta_generic_to_shared(lutb + 65536) + warp * (D * kRingStageBytes);
             const uint32_t per_stage = 32 * NBS;
             const uint32_t n_st = (U + kScanWarps * per_stage - 1) / (kScanWarps * per_stage);   // stages per warp
-            uint32_t idn[NBS];                                 // IDs of the next stage to issue, loaded one stage ahead
+            uint32_t idn[NBS], kidn[NBS];                      // rows of the next stage to issue and their vector-IDs, loaded one stage ahead
             auto load_ids = [&](uint32_t st) {
                 const uint32_t base = (st * kScanWarps + warp) * per_stage;
 #pragma unroll
                 for (int nb = 0; nb < NBS; ++nb) {
                     const uint32_t idx = base + nb * 32 + lane;
-                    idn[nb] = idx < U ? __ldg(uq + idx) : kIdNone;
+                    if constexpr (LM) {                        // (row of the list-major copy, vector-ID) pairs
+                        const uint2 rv = idx < U ? __ldg(reinterpret_cast<const uint2 *>(p.key_src) + off0 + idx)
+                                                 : make_uint2(kIdNone, kIdNone);
+                        idn[nb] = rv.x; kidn[nb] = rv.y;
+                    } else {
+                        idn[nb] = idx < U ? __ldg(uq + idx) : kIdNone;
+                        kidn[nb] = idn[nb];
+                    }
                 }
             };
             // start the copies of stage st (its IDs are in idn), then fetch the IDs of stage st + 1
@@ -1070,7 +1169,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                     const uint32_t sa = ring + (st % D) * kRingStageBytes;
 #pragma unroll
                     for (int nb = 0; nb < NBS; ++nb) {
-                        sts_u32(sa + 2048 + (nb * 32 + lane) * 4, idn[nb]);
+                        sts_u32(sa + 2048 + (nb * 32 + lane) * 4, kidn[nb]);
 #pragma unroll
                         for (int t = 0; t < G; ++t) {
                             uint32_t rid = G == 1 ? idn[nb] : __shfl_sync(0xffffffffu, idn[nb], (lane & ~(G - 1)) | t);
@@ -1112,7 +1211,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                             }
                             const uint32_t idv = lds_u32(sa + 2048 + (nb * 32 + lane) * 4);
                             const unsigned long long key = ((unsigned long long)__float_as_uint(mine) << 32) | idv;
-                            const bool keep = idv != kIdNone && key < tau;
+                            const bool keep = (LM ? idv < p.id_limit : idv != kIdNone) && key < tau;
                             const uint32_t bal = __ballot_sync(0xffffffffu, keep);
                             if (bal) {
                                 uint32_t pos = 0;
@@ -1127,7 +1226,8 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
                     ++st;
                 }
                 if (!__syncthreads_or(vm[9] != 0)) break;
-                prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
+                if constexpr (LM) { prune_exact(buf, misc, rank, p.k, p.cap); if (tid == 0) misc[9] = 0; __syncthreads(); }
+                else prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
             }
             cp_async_wait<0>();
         } else {
@@ -1193,15 +1293,20 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 
         // exact top-k of what is left
         uint32_t n = vm[0];
-        if (n > 2 * p.k && n >= 1024) {
-            prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
+        if constexpr (LM) {                                    // list-major experiment: sorted and free of repeats
+            prune_exact(buf, misc, rank, p.k, p.cap);
             n = vm[0];
+        } else {
+            if (n > 2 * p.k && n >= 1024) {
+                prune<KPT>(buf, misc, samp, rank, p.k, p.cap, limit);
+                n = vm[0];
+            }
+            uint32_t P = 32;
+            while (P < n) P <<= 1;
+            for (uint32_t i = n + tid; i < P; i += kScanThreads) buf[i] = kKeyMax;
+            __syncthreads();
+            bitonic_sort_smem(buf, P, 2);
         }
-        uint32_t P = 32;
-        while (P < n) P <<= 1;
-        for (uint32_t i = n + tid; i < P; i += kScanThreads) buf[i] = kKeyMax;
-        __syncthreads();
-        bitonic_sort_smem(buf, P, 2);
         const uint32_t cnt = n < p.k ? n : p.k;
         if (p.parts > 1) {                                     // partial result: the slice's k smallest keys, padded
             unsigned long long *pk = p.part_keys + ((size_t)b * p.parts + part) * p.k;

@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(kExpandThreads) lists_expand_kernel(const long
                                                                       const uint32_t *__restrict__ probes, uint32_t nprobe,
                                                                       const long long *__restrict__ cand_offsets,
                                                                       uint32_t *__restrict__ cand_ids, const ListsHeader *hdr,
-                                                                      uint32_t ctas_per_query)
+                                                                      uint32_t ctas_per_query, uint32_t write_rows)
 {
     extern __shared__ uint32_t start[];                           // [nprobe + 1] positions inside the query's list
     __shared__ uint32_t carry;
@@ -135,10 +135,32 @@ __global__ void __launch_bounds__(kExpandThreads) lists_expand_kernel(const long
     for (uint32_t j = sub * (kExpandThreads / 32) + warp; j < nprobe; j += ctas_per_query * (kExpandThreads / 32)) {
         const uint32_t len = start[j + 1] - start[j];
         if (!len) continue;
-        const uint32_t *src = list_ids + __ldg(list_offsets + __ldg(pr + j));
+        const long long l0 = __ldg(list_offsets + __ldg(pr + j));
+        const uint32_t *src = list_ids + l0;
         uint32_t *dst = out + start[j];
+        if (write_rows) {
+            // list-major experiment: (the entry's position in list_ids = the row of the list-major code copy, its vector-ID)
+            uint2 *dst2 = reinterpret_cast<uint2 *>(cand_ids) + cand_offsets[b] + start[j];
+            for (uint32_t e = lane; e < len; e += 32) dst2[e] = make_uint2((uint32_t)l0 + e, __ldg(src + e));
+            continue;
+        }
         for (uint32_t e = lane; e < len; e += 32) dst[e] = __ldg(src + e);
     }
+}
+
+// List-major experiment: row e of the copy = the code row of the vector list entry e names (zero if it names none).
+__global__ void list_codes_kernel(const uint8_t *__restrict__ codes, uint64_t N, uint32_t row_bytes,
+                                  const uint32_t *__restrict__ list_ids, uint64_t e0, uint64_t n, uint8_t *__restrict__ dst)
+{
+    const uint32_t chunks = row_bytes >> 4;
+    const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n * chunks) return;
+    const uint64_t e = e0 + t / chunks;
+    const uint32_t c = (uint32_t)(t % chunks);
+    const uint32_t id = __ldg(list_ids + e);
+    uint4 v = make_uint4(0, 0, 0, 0);
+    if ((uint64_t)id < N) v = __ldg(reinterpret_cast<const uint4 *>(codes + (uint64_t)id * row_bytes) + c);
+    reinterpret_cast<uint4 *>(dst + e * row_bytes)[c] = v;
 }
 
 // ---------------------------------------------------------------- (8) heuristic re-ranking, Algorithm 1

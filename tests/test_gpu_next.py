@@ -155,6 +155,89 @@ def test_search_lists_full_size_equals_id_path(fann):
     ix.close()
 
 
+# ------------------------------------------------------------------ experiment: list-major code copy, streamed
+
+def _search_stream(fann, ix, w, probes_np, k, cap):
+    B = probes_np.shape[0]
+    lut = ix.build_lut(w.queries[:B].contiguous().to(DEV), w.codebooks.to(DEV))
+    need = fann.fann_search_lists_stream_workspace_bytes(ix.handle, B, cap)
+    ws = torch.empty(need, dtype=torch.uint8, device=DEV)
+    oi = torch.empty((B, k), dtype=torch.int32, device=DEV)
+    od = torch.empty((B, k), dtype=torch.float32, device=DEV)
+    oc = torch.empty(B, dtype=torch.int32, device=DEV)
+    st = torch.cuda.current_stream().cuda_stream
+    fann.fann_search_lists_stream(ix.handle, lut, B, as_dev_u32(probes_np), probes_np.shape[1], cap, k, oi, od, oc, ws, need, st)
+    total = fann.fann_search_lists_stream_status(ix.handle, ws, st)
+    return np_u32(oi), od.cpu().numpy(), np_u32(oc), total
+
+
+@pytest.mark.parametrize("k", [1, 100, 1000])
+def test_list_major_stream_gives_the_oracles_bytes(fann, wl_int, k):
+    """Every candidate is scored, repeats included, and the repeats leave where the top-k buffer is pruned: same
+    ids / dists / counts as the oracle (integer data: bytes), also with padding probes, a list named twice (every ID
+    of it twice), unknown lists and an empty query."""
+    w = wl_int
+    ix = _index_with_lists(fann, w)
+    fann.fann_build_list_codes(ix.handle)
+    P = w.probes.numpy().view(np.uint32).copy()
+    P[0, ::2] = NONE
+    P[1, :5] = w.cfg.n_lists + 7
+    P[2, :] = NONE
+    P[3, 1::2] = P[3, 0::2]                                      # every second probe repeats its neighbour
+    cap = w.cand_ids.numel() + 1000
+    gi, gd, gc, total = _search_stream(fann, ix, w, P, k, cap)
+    ref = oracle.search_lists(w.queries.numpy(), w.codebooks.numpy(), w.codes.numpy(), w.list_offsets.numpy(),
+                              w.list_ids.numpy(), P, k)
+    assert np.array_equal(gi, ref["ids"]) and np.array_equal(gd.view(np.uint32), ref["dists"].view(np.uint32))
+    assert np.array_equal(gc, ref["counts"]) and gc[2] == 0
+    assert total == int(oracle.expand_lists(w.list_offsets.numpy(), w.list_ids.numpy(), P)[0][-1])
+    with pytest.raises(fann.FannError) as err:                   # a workspace sized for fewer candidates: refused
+        _search_stream(fann, ix, w, P, k, total - 1)
+    assert err.value.code == -5 and err.value.total_cands == total
+    ix.close()
+
+
+def test_list_major_stream_fp32_band(fann, wl_tiny):
+    w = wl_tiny
+    ix = _index_with_lists(fann, w)
+    fann.fann_build_list_codes(ix.handle)
+    P = w.probes.numpy().view(np.uint32)
+    gi, gd, gc, _ = _search_stream(fann, ix, w, P, w.cfg.k, w.cand_ids.numel())
+    off, ids = oracle.expand_lists(w.list_offsets.numpy(), w.list_ids.numpy(), P)
+    for b in range(w.cfg.B):
+        ai, ad = oracle.query_all(w.queries.numpy()[b], w.codebooks.numpy(), w.codes.numpy(), ids[off[b]:off[b + 1]])
+        check_band(gi[b], gd[b], gc[b], ai, ad, w.cfg.k)
+    ix.close()
+
+
+def test_list_major_stream_heavy_repeats(fann):
+    """Few distinct vectors, each many times: one short list probed 300 times, k below and above the distinct count
+    (the buffer fills with repeats many times over and must still end with each vector once)."""
+    rng = np.random.default_rng(11)
+    N, M, dsub = 5_000, 32, 4
+    codes = rng.integers(0, 256, size=(N, M), dtype=np.uint8)
+    cb = rng.integers(0, 256, size=(M, 256, dsub)).astype(np.float32)
+    q = rng.integers(0, 256, size=(2, M * dsub)).astype(np.float32)
+    lists = [rng.choice(N, 40, replace=False).astype(np.uint32), rng.choice(N, 2000, replace=False).astype(np.uint32)]
+    loff = np.array([0, 40, 2040], np.int64)
+    lids = np.concatenate(lists)
+    P = np.zeros((2, 300), np.uint32)
+    P[1, ::3] = 1                                                # query 1: both lists, 200 and 100 times
+    ix = fann.FannIndex(0)
+    ix.load_codes(torch.from_numpy(codes).to(DEV))
+    ix.load_lists(torch.from_numpy(loff).to(DEV), torch.from_numpy(lids.view(np.int32)).to(DEV))
+    fann.fann_build_list_codes(ix.handle)
+
+    class W:                                                     # what _search_stream reads
+        queries, codebooks = torch.from_numpy(q), torch.from_numpy(cb)
+    for k in (10, 64, 1024):
+        gi, gd, gc, total = _search_stream(fann, ix, W, P, k, 300 * 2040)
+        ref = oracle.search_lists(q, cb, codes, loff, lids, P, k)
+        assert np.array_equal(gi, ref["ids"]) and np.array_equal(gd.view(np.uint32), ref["dists"].view(np.uint32))
+        assert np.array_equal(gc, ref["counts"])
+    ix.close()
+
+
 # ------------------------------------------------------------------ NEXT-1: heuristic re-ranking (Algorithm 1)
 
 def _pq_stage_tasks(fann, w, n):
