@@ -92,3 +92,19 @@ def test_feistel_id_map_is_a_bijection_that_scatters():
     assert np.unique(gaps).size > 1000
     y2 = feistel_permute(t, N, key=8).numpy()
     assert not np.array_equal(np.sort(y2), y)                    # keyed
+
+
+def test_bench_reads_the_committed_dram_traffic():
+    """roofline.traffic comes from the ncu launch lists committed under profiles/ (not a typed-in constant): every
+    large workload has an entry for the dominant kernel, within a few percent of the kernel's algorithmic bytes."""
+    import bench
+    from workloads import CONFIGS
+    for name, U in (("u8_1b_m64", 732_249_656),):
+        t, src = bench.traffic_from_profiles(name, "scan_kernel")
+        cfg = CONFIGS[name]
+        algo = cfg.M * U + 4 * U + 1024 * cfg.M * cfg.B + 8 * cfg.k * cfg.B
+        assert src and abs(t - algo) < 0.02 * algo
+    for name in ("i8_1b_m25", "f32_100m_m48", "u8_10m_m32"):
+        t, src = bench.traffic_from_profiles(name, "scan_kernel")
+        assert t and t > 0 and src
+    assert bench.traffic_from_profiles("tiny", "scan_kernel") == (None, None)
