@@ -135,6 +135,7 @@ struct Geom {
     uint32_t nslots_max, cap_c, dedup_smem, dedup_threads;   // dedup: table slots per CTA, candidates per partition, CTA shape
     uint32_t cap, scan_smem, ring;                   // scan: candidate-buffer keys, shared memory per CTA, ring depth
     uint32_t parts, k;                               // scan CTAs per query (> 1 for batches smaller than the machine), k
+    uint32_t part_ctas;                              // partition CTAs per query (> 1 for small batches)
 };
 
 // Dedup CTA shape: one 1024-thread CTA per SM with the whole shared memory as its table, or -- when the mean candidate
@@ -163,12 +164,15 @@ static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t tota
         const uint32_t fit = (uint32_t)ix->num_sms / B;
         g->parts = fit >= 16 ? 16u : fit >= 8 ? 8u : fit >= 4 ? 4u : 2u;   // a power of two (pairwise merge)
     }
+    g->part_ctas = 1;
+    if (ix->split_scan && allow_split)
+        while (g->part_ctas < 16 && 2 * g->part_ctas * B <= (uint32_t)ix->num_sms) g->part_ctas <<= 1;
     g->cap = (k <= 256 || g->ring) ? 4096u : 8192u;            // the ring takes the shared memory of the larger buffer
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap, g->ring);
 }
 
 struct WsLayout {
-    size_t hdr, S, mode, item_start, items, uniq_counts, part_ok, bucket_cnt, part_keys, part_ids, uniq_ids, total;
+    size_t hdr, S, mode, item_start, items, uniq_counts, part_ok, part_aux, bucket_cnt, part_keys, part_ids, uniq_ids, total;
     uint32_t max_items;
 };
 
@@ -184,6 +188,7 @@ static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with
     w->items = o;       o = align_up(o + (size_t)w->max_items * 8, 256);
     w->uniq_counts = o; o = align_up(o + (size_t)B * 4, 256);
     w->part_ok = o;     o = align_up(o + (size_t)B * 4, 256);
+    w->part_aux = o;    o = align_up(o + (size_t)B * 8, 256);        // partition_multi_kernel: arrivals, failure flag
     w->bucket_cnt = o;  o = align_up(o + (size_t)w->max_items * 4, 256);
     w->part_keys = o;   if (g.parts > 1) o = align_up(o + (size_t)B * g.parts * g.k * 8, 256);   // partial top-k of the scan parts
     w->part_ids = o;    o = align_up(o + (size_t)total_cands * 8 + 16, 256);      // class buckets, 2 C_b per query
@@ -482,7 +487,9 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     if (timing) cudaEventRecord(ix->ev_plan[0], stream);
     plan_kernel<<<1, 1024, 0, stream>>>((const long long *)cand_offsets, B, g.cap_c, w.max_items, hdr, S,
                                         item_start, items, uniq_counts, keep_status ? 1u : 0u,
-                                        (unsigned long long)total_cands, exact_total ? 1u : 0u);
+                                        (unsigned long long)total_cands, exact_total ? 1u : 0u,
+                                        g.part_ctas > 1 ? (uint32_t *)(ws + w.bucket_cnt) : nullptr,
+                                        g.part_ctas > 1 ? (uint32_t *)(ws + w.part_aux) : nullptr);
     mode_kernel<<<(B + 7) / 8, 256, 0, stream>>>((const long long *)cand_offsets, cand_ids, B, ix->N,
                                                   ix->force_mode, ix->partition ? 0u : g.cap_c, mode);
     if (timing) cudaEventRecord(ix->ev_plan[1], stream);
@@ -512,6 +519,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     pp.part_ids = (uint32_t *)(ws + w.part_ids); pp.part_ok = (uint32_t *)(ws + w.part_ok);
     pp.bucket_cnt = (uint32_t *)(ws + w.bucket_cnt);
     pp.class_max = (uint32_t)((uint64_t)g.nslots_max * 9 / 10);
+    pp.ctas = g.part_ctas; pp.aux = (uint32_t *)(ws + w.part_aux);
     ScanParams sp;
     sp.codes = ix->codes; sp.M = ix->M; sp.lut = lut; sp.cand_offsets = (const long long *)cand_offsets;
     sp.uniq_ids = uniq_ids; sp.uniq_counts = uniq_counts; sp.k = k; sp.cap = g.cap;
@@ -542,7 +550,8 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         if (!overlap && ix->partition && c == 0) {
             pp.q_begin = 0;
             if (timing) cudaEventRecord(ix->ev_part[0], stream);
-            partition_kernel<<<B, kPartThreads, 0, stream>>>(pp);
+            if (g.part_ctas > 1) partition_multi_kernel<<<B * g.part_ctas, kPartThreads, 0, stream>>>(pp);
+            else partition_kernel<<<B, kPartThreads, 0, stream>>>(pp);
             if (timing) { cudaEventRecord(ix->ev_part[1], stream); ix->have_part = true; }
             ix->launches++;
             CUDA_TRY(cudaGetLastError());
@@ -790,12 +799,11 @@ extern "C" size_t fann_search_lists_workspace_bytes(const fann_index *ix, uint32
     return l.total;
 }
 
-// Steps (3)(5)(6)(7) for B queries inside a workspace laid out by `l` (which may have been sized for a larger batch of
-// which these queries are a chunk: every region is used from its start).
+// Steps (3)(5)(6)(7) for B queries inside a workspace laid out by `l`.
 static int search_lists_impl(fann_index *ix, const float *lut, uint32_t B, const uint32_t *probes, uint32_t nprobe,
                              uint64_t max_total_cands, uint32_t k, uint32_t *out_ids, float *out_dists,
                              uint32_t *out_counts, uint32_t *out_uniq, char *ws, const ListsLayout &l,
-                             cudaStream_t stream, bool later_chunk, bool allow_split, uint32_t shape = 0)
+                             cudaStream_t stream)
 {
     ListsHeader *hdr = (ListsHeader *)(ws + l.hdr);
     long long *offsets = (long long *)(ws + l.offsets);
@@ -803,7 +811,7 @@ static int search_lists_impl(fann_index *ix, const float *lut, uint32_t B, const
     lists_count_kernel<<<(B + 7) / 8, 256, 0, stream>>>(ix->list_offsets, ix->n_lists, probes, B, nprobe,
                                                          (unsigned long long *)offsets);
     lists_scan_kernel<<<1, 1024, 0, stream>>>((const unsigned long long *)offsets, B, offsets, hdr,
-                                              (unsigned long long)max_total_cands, later_chunk ? 1u : 0u);
+                                              (unsigned long long)max_total_cands);
     uint32_t expand_ctas = 1;                                  // small batches: spread a query's lists over several CTAs
     while (expand_ctas < 16 && 2 * expand_ctas * B <= (uint32_t)ix->num_sms && 8 * expand_ctas < nprobe) expand_ctas <<= 1;
     lists_expand_kernel<<<B * expand_ctas, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(
@@ -812,7 +820,7 @@ static int search_lists_impl(fann_index *ix, const float *lut, uint32_t B, const
     CUDA_TRY(cudaGetLastError());
     // a batch larger than the workspace was sized for leaves cand_offsets[B] > max_total_cands: the path refuses it
     return run_path(ix, false, lut, B, (const int64_t *)offsets, ids, max_total_cands, k, out_ids, out_dists, out_counts,
-                    out_uniq, nullptr, nullptr, ws + l.ws, l.ws_bytes, stream, shape, later_chunk, false, allow_split);
+                    out_uniq, nullptr, nullptr, ws + l.ws, l.ws_bytes, stream, 0, false, false);
 }
 
 extern "C" int fann_search_lists(fann_index *ix, const float *lut, uint32_t B, const uint32_t *probes, uint32_t nprobe,
@@ -833,7 +841,7 @@ extern "C" int fann_search_lists(fann_index *ix, const float *lut, uint32_t B, c
     if (workspace_bytes < l.total) return fail(FANN_EWORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, l.total);
     DeviceGuard guard(ix->device);
     return search_lists_impl(ix, lut, B, probes, nprobe, max_total_cands, k, out_ids, out_dists, out_counts, out_uniq,
-                             (char *)workspace, l, (cudaStream_t)stream_, false, true);
+                             (char *)workspace, l, (cudaStream_t)stream_);
 }
 
 extern "C" int fann_search_lists_status(fann_index *ix, const void *workspace, uint32_t B, uint64_t max_total_cands,
@@ -908,41 +916,19 @@ extern "C" int fann_search_lists_host(fann_index *ix, const float *queries_h, ui
     CUDA_TRY(cudaMemcpyAsync(s + h.probes, probes_h, (size_t)B * nprobe * 4, cudaMemcpyHostToDevice, stream));
     int rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
     if (rc != FANN_OK) return rc;
-    // The batch can run in chunks of queries, a chunk's results going down on a second stream while the next chunk
-    // computes.  Measured at u8_1b_m64 (80 MB of results, 1.4 ms of PCIe time): 4 chunks cost more in kernel ramp-up
-    // and drain (4.1 ms over the device path) than the overlap saves (2.9 ms in one piece), so one chunk it is.
-    const uint32_t nchunk = 1u;
+    // (Running the batch in chunks of queries, a chunk's results going down on a second stream while the next chunk
+    // computes, was measured at u8_1b_m64 -- 80 MB of results, 1.4 ms of PCIe time: 4 chunks cost more in kernel
+    // ramp-up and drain, 4.1 ms over the device path, than the overlap saves, 2.9 ms in one piece.)
     ListsLayout l;
     lists_layout(ix, B, max_total_cands, k, &l);
-    Geom g;
-    geometry(ix, k, B, max_total_cands, &g);                   // one dedup CTA shape for all chunks: the layout depends on it
-    CtxLease lease(nchunk > 1 ? ix : nullptr);
-    CallCtx *cx = lease.c;
-    if (nchunk > 1 && !cx) return fail(FANN_ECUDA, "fann_search_lists_host: could not create the transfer stream");
-    for (uint32_t c = 0; c < nchunk; ++c) {
-        const uint32_t b0 = (uint32_t)((uint64_t)B * c / nchunk), b1 = (uint32_t)((uint64_t)B * (c + 1) / nchunk);
-        uint32_t *oi = (uint32_t *)(s + h.out_ids) + (size_t)b0 * k;
-        float *od = (float *)(s + h.out_dists) + (size_t)b0 * k;
-        uint32_t *oc = (uint32_t *)(s + h.out_counts) + b0;
-        rc = search_lists_impl(ix, (const float *)(s + h.lut) + (size_t)b0 * ix->M * 256, b1 - b0,
-                               (const uint32_t *)(s + h.probes) + (size_t)b0 * nprobe, nprobe, max_total_cands, k, oi, od, oc,
-                               nullptr, s + h.ws, l, stream, c > 0, nchunk == 1, nchunk > 1 ? g.dedup_threads : 0u);
-        if (rc != FANN_OK) return rc;
-        cudaStream_t down = stream;
-        if (nchunk > 1) {
-            CUDA_TRY(cudaEventRecord(cx->ev_done[c], stream));
-            CUDA_TRY(cudaStreamWaitEvent(cx->side, cx->ev_done[c], 0));
-            down = cx->side;
-        }
-        CUDA_TRY(cudaMemcpyAsync(out_ids_h + (size_t)b0 * k, oi, (size_t)(b1 - b0) * k * 4, cudaMemcpyDeviceToHost, down));
-        CUDA_TRY(cudaMemcpyAsync(out_dists_h + (size_t)b0 * k, od, (size_t)(b1 - b0) * k * 4, cudaMemcpyDeviceToHost, down));
-        if (out_counts_h)
-            CUDA_TRY(cudaMemcpyAsync(out_counts_h + b0, oc, (size_t)(b1 - b0) * 4, cudaMemcpyDeviceToHost, down));
-    }
-    if (nchunk > 1) {
-        CUDA_TRY(cudaEventRecord(cx->ev_fork, cx->side));
-        CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_fork, 0));     // `stream` ends after the last copy
-    }
+    rc = search_lists_impl(ix, (const float *)(s + h.lut), B, (const uint32_t *)(s + h.probes), nprobe, max_total_cands, k,
+                           (uint32_t *)(s + h.out_ids), (float *)(s + h.out_dists), (uint32_t *)(s + h.out_counts), nullptr,
+                           s + h.ws, l, stream);
+    if (rc != FANN_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+    CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+    if (out_counts_h)
+        CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
     return fann_search_lists_status(ix, s + h.ws, B, max_total_cands, k, nullptr, stream);   // synchronises
 }
 
@@ -1028,7 +1014,7 @@ extern "C" int fann_search_lists_stream(fann_index *ix, const float *lut, uint32
     lists_count_kernel<<<(B + 7) / 8, 256, 0, stream>>>(ix->list_offsets, ix->n_lists, probes, B, nprobe,
                                                          (unsigned long long *)offsets);
     lists_scan_kernel<<<1, 1024, 0, stream>>>((const unsigned long long *)offsets, B, offsets, hdr,
-                                              (unsigned long long)max_total_cands, 0u);
+                                              (unsigned long long)max_total_cands);
     lists_expand_kernel<<<B, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(
         ix->list_offsets, ix->list_ids, ix->n_lists, probes, nprobe, offsets, rows, hdr, 1u, 1u);
     stream_counts_kernel<<<(B + 255) / 256, 256, 0, stream>>>(offsets, B, counts, counter, hdr);

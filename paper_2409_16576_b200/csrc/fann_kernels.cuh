@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(256) build_lut_kernel(const float *__restrict_
 __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t B, uint32_t cap_c,
                             uint32_t max_items, WsHeader *hdr, uint32_t *S, uint32_t *item_start,
                             uint2 *items, uint32_t *uniq_counts, uint32_t keep_status,
-                            unsigned long long total_cands, uint32_t exact_total)
+                            unsigned long long total_cands, uint32_t exact_total, uint32_t *bucket_cnt, uint32_t *part_aux)
 {
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t running;
@@ -215,6 +215,7 @@ __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t
             if (refuse) s = 0;                                 // no partition, no dedup item; the scan sees U = 0
             S[b] = s;
             uniq_counts[b] = 0;
+            if (part_aux) { part_aux[2 * b] = 0; part_aux[2 * b + 1] = 0; }   // partition_multi_kernel: arrivals, failure
         }
         uint32_t incl = s;                                     // block inclusive scan
         for (int o = 1; o < 32; o <<= 1) {
@@ -236,7 +237,7 @@ __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t
         if (b < B) {
             item_start[b] = start;
             for (uint32_t p = 0; p < s; ++p)
-                if (start + p < max_items) items[start + p] = make_uint2(b, p);
+                if (start + p < max_items) { items[start + p] = make_uint2(b, p); if (part_aux) bucket_cnt[start + p] = 0; }
         }
         __syncthreads();
         if (threadIdx.x == blockDim.x - 1) running = start + s;
@@ -366,6 +367,8 @@ struct PartParams {
     uint32_t *bucket_cnt;                            // [n_items]
     uint32_t q_begin;                                // first query of this launch (one CTA per query)
     uint32_t class_max;                              // most IDs of one class a dedup table takes if none repeats (90 % load)
+    uint32_t ctas;                                   // partition_multi_kernel: CTAs per query (small batches)
+    uint32_t *aux;                                   // partition_multi_kernel: [B][2] arrivals, failure flag (zeroed per call)
 };
 
 // Splits the candidate list of every query that needs S >= 2 dedup partitions into its S classes, so that
@@ -457,6 +460,100 @@ __global__ void __launch_bounds__(kPartThreads) partition_kernel(const PartParam
         if (tid < S) p.bucket_cnt[p.item_start[b] + tid] = scnt[tid] < capb ? scnt[tid] : capb;
         if (tid == 0) p.part_ok[b] = bad ? 0u : 1u;
         return;
+    }
+}
+
+// Small batches: the same split with p.ctas CTAs per query, so that one query's list does
+// not wait on one SM.  Every CTA takes a slice of the list: it counts its IDs per class, reserves each class's range
+// in the query's bucket with one global atomic per class (bucket_cnt is the cursor and ends as the class total), then
+// scatters.  The query's last CTA to finish closes it: buckets valid, or -- a class overflowed its bucket or would
+// overfill a dedup table -- not valid and the query switched to hash classes, which the dedup kernel then filters
+// from the original list (the one-CTA kernel splits such a query again instead; here it is the rare case).
+__global__ void __launch_bounds__(kPartThreads) partition_multi_kernel(const PartParams p)
+{
+    __shared__ uint32_t scnt[kMaxPartBuckets];
+    __shared__ uint32_t s_last;
+    const uint32_t b = p.q_begin + blockIdx.x / p.ctas, sub = blockIdx.x % p.ctas;
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    const uint32_t scnt_addr = (uint32_t)__cvta_generic_to_shared(scnt);
+    const uint32_t S = p.S[b];
+    if (S < 2 || S > kMaxPartBuckets) {
+        if (sub == 0 && tid == 0) { p.part_ok[b] = 0; if (S > kMaxPartBuckets) p.mode[b] = kModeHashed; }
+        return;
+    }
+    const bool hashed = p.mode[b] == kModeHashed;              // nobody changes it before every CTA of the query has read it
+    const long long off0 = p.cand_offsets[b];
+    const long long Cll = p.cand_offsets[b + 1] - off0;
+    const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;
+    const uint32_t capb = (uint32_t)(2ull * C / S);
+    uint32_t *out = p.part_ids + 2 * off0;
+    const uint32_t *ids = p.cand_ids + off0;
+    const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
+    const uint32_t nvec = (C + shift + 3u) >> 2;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const uint4 *ids4 = reinterpret_cast<const uint4 *>(ids - shift);
+    const uint32_t v_in0 = shift ? 1u : 0u, v_in1 = (C + shift) >> 2;
+    auto load_vec = [&](uint32_t v) -> uint4 {
+        if (v >= v_in0 && v < v_in1) return __ldg(ids4 + v);
+        if (v < nvec) return load_ids4(ids, 4ll * v - shift, C);
+        return make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+    };
+    const uint32_t v_lo = (uint32_t)((unsigned long long)nvec * sub / p.ctas);
+    const uint32_t v_hi = (uint32_t)((unsigned long long)nvec * (sub + 1) / p.ctas);
+    const uint32_t N32 = (uint32_t)p.N;
+    const uint32_t MS = hashed ? 0u : ordered_class_mul(p.N, S);
+    auto class_of = [&](uint32_t x) -> uint32_t {
+        if (x >= N32) return 0xFFu;                            // also kIdNone
+        return hashed ? __umulhi(hash_round1(x), S) : __umulhi(x, MS);
+    };
+    if (tid < kMaxPartBuckets) scnt[tid] = 0;
+    if (tid == 0) s_last = 0;
+    __syncthreads();
+    uint32_t overflow = 0;
+    for (int pass = 0; pass < 2; ++pass) {                     // 0: count, 1: scatter (the slice is in L2 by then)
+        for (uint32_t vb = v_lo; vb < v_hi; vb += kPartThreads) {   // uniform trip count: the matches need whole warps
+            const uint4 q4 = vb + tid < v_hi ? load_vec(vb + tid) : make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+            const uint32_t x[4] = {q4.x, q4.y, q4.z, q4.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const uint32_t cls = class_of(x[e]);
+                const uint32_t own = __match_any_sync(0xffffffffu, cls);
+                const uint32_t leader = __ffs(own) - 1;
+                uint32_t base = 0;
+                if (cls != 0xFFu && lane == leader) base = atoms_add(scnt_addr + (cls << 2), (uint32_t)__popc(own));
+                if (pass) {
+                    base = __shfl_sync(0xffffffffu, base, leader);
+                    const uint32_t pos = base + __popc(own & lt_mask);
+                    if (cls != 0xFFu) {
+                        if (pos < capb) out[cls * capb + pos] = x[e];
+                        else overflow = 1;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        if (!pass) {                                           // this CTA's range in every class's bucket
+            if (tid < S) scnt[tid] = atomicAdd(&p.bucket_cnt[p.item_start[b] + tid], scnt[tid]);
+            __syncthreads();
+        }
+    }
+    if (__syncthreads_or(overflow != 0) && tid == 0) atomicOr(&p.aux[2 * b + 1], 1u);
+    if (tid == 0) {
+        __threadfence();
+        s_last = atomicAdd(&p.aux[2 * b], 1u) == p.ctas - 1 ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    bool bad = *reinterpret_cast<volatile uint32_t *>(&p.aux[2 * b + 1]) != 0;
+    uint32_t total = 0;
+    if (tid < S) total = *reinterpret_cast<volatile uint32_t *>(&p.bucket_cnt[p.item_start[b] + tid]);
+    if (!hashed) bad = bad || total > p.class_max;             // would overfill a dedup table if none of its IDs repeats
+    bad = __syncthreads_or(bad);
+    if (tid < S && total > capb) p.bucket_cnt[p.item_start[b] + tid] = capb;
+    if (tid == 0) {
+        p.part_ok[b] = bad ? 0u : 1u;
+        if (bad && !hashed) p.mode[b] = kModeHashed;
     }
 }
 

@@ -15,10 +15,10 @@ namespace fann {
 // ---------------------------------------------------------------- (3) candidate lists from resident metadata
 
 struct ListsHeader {                                  // first 64 bytes of a fann_search_lists workspace
-    unsigned long long total;                         // sum of the probed lists' lengths of the batch (of its largest chunk)
+    unsigned long long total;                         // sum of the probed lists' lengths of the batch
     unsigned long long capacity;                      // max_total_cands of the call
     uint32_t overflow;                                // 1: total > capacity, nothing was expanded
-    uint32_t pad[11];                                 // [0]: this chunk alone exceeds the capacity
+    uint32_t pad[11];
 };
 
 // One warp per query: C_b = sum of the lengths of its probed lists.  A probe equal to 0xFFFFFFFF is padding and a
@@ -42,7 +42,7 @@ __global__ void lists_count_kernel(const long long *__restrict__ list_offsets, u
 // Single CTA: cand_offsets[b] = exclusive prefix sum of per_query (in place: per_query and cand_offsets may be the
 // same array of B + 1 entries), total and the capacity check into the header.
 __global__ void lists_scan_kernel(const unsigned long long *per_query, uint32_t B, long long *cand_offsets,
-                                  ListsHeader *hdr, unsigned long long capacity, uint32_t later_chunk)
+                                  ListsHeader *hdr, unsigned long long capacity)
 {
     __shared__ unsigned long long warp_sums[32];
     __shared__ unsigned long long running;
@@ -77,13 +77,9 @@ __global__ void lists_scan_kernel(const unsigned long long *per_query, uint32_t 
     }
     if (threadIdx.x == 0) {
         cand_offsets[B] = (long long)running;
-        // a later chunk of the same batch (fann_search_lists_host) keeps what the earlier chunks reported; `chunk_over`
-        // tells this chunk's expansion whether to run
-        const uint32_t over = running > capacity ? 1u : 0u;
-        hdr->total = later_chunk ? (hdr->total > running ? hdr->total : running) : running;
+        hdr->total = running;
         hdr->capacity = capacity;
-        hdr->overflow = (later_chunk ? hdr->overflow : 0u) | over;
-        hdr->pad[0] = over;
+        hdr->overflow = running > capacity ? 1u : 0u;
     }
 }
 
@@ -100,7 +96,7 @@ __global__ void __launch_bounds__(kExpandThreads) lists_expand_kernel(const long
 {
     extern __shared__ uint32_t start[];                           // [nprobe + 1] positions inside the query's list
     __shared__ uint32_t carry;
-    if (hdr->pad[0]) return;                                      // the workspace cannot hold this chunk: write nothing
+    if (hdr->overflow) return;                                    // the workspace cannot hold the batch: write nothing
     // small batches: several CTAs per query share its lists (CTA `sub` copies lists sub * 8 + warp, + 8 * ctas, ...)
     const uint32_t b = blockIdx.x / ctas_per_query, sub = blockIdx.x - b * ctas_per_query;
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
