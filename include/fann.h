@@ -291,7 +291,11 @@ int fann_search_lists_stream_status(fann_index *ix, const void *workspace, uint6
  * threads may call concurrently on one index and one pool; calls share no workspace, stream
  * or event.  A batch of fewer queries than half the SMs is scanned by several CTAs per query
  * (each on a slice of the query's distinct list, merged on the device), so that one query
- * does not wait on one SM; results are the same bytes as the batched entry points give.
+ * does not wait on one SM -- and so are its list expansion and its partition pass; results are
+ * the same bytes as the batched entry points give.  fann_search_small_lists replays ONE CUDA
+ * graph per call (captured per block and call shape -- B, nprobe, k, codebooks -- on first use):
+ * the inputs are copied into the block's pinned staging buffer, the graph copies them up, runs
+ * the ten kernels and copies results and status back (FANN_SMALL_GRAPH=0: plain launches).
  * Errors: EINVAL (NULL, a pool of another index, B / k / dsub / nprobe outside what the pool
  * was created for), EWORKSPACE (more candidate IDs than a block holds), and what the batched
  * entry points return.

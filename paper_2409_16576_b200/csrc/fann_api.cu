@@ -1062,6 +1062,13 @@ struct fann_pool {
     uint32_t n_blocks = 0, max_B = 0, k_max = 0, dsub = 0, max_nprobe = 0;
     uint64_t max_cands = 0;
     std::vector<cudaStream_t> streams;
+    // CUDA graphs of the posting-list form (one per block and call shape): the ten kernel launches and five copies of
+    // a call replayed by one cudaGraphLaunch from the block's pinned staging buffer
+    struct Graph { uint32_t B, nprobe, k; const float *codebooks; cudaGraphExec_t exec; };
+    std::vector<std::vector<Graph>> graphs;        // per block; a block is used by one call at a time
+    char *staging = nullptr;                       // pinned host memory, staging_bytes per block
+    size_t staging_bytes = 0, st_queries = 0, st_probes = 0, st_ids = 0, st_dists = 0, st_counts = 0, st_hdr = 0;
+    bool use_graphs = true;                        // FANN_SMALL_GRAPH=0: plain launches
     std::mutex mu;
     std::condition_variable cv;
     std::vector<uint32_t> free_blocks;
@@ -1087,6 +1094,7 @@ struct BlockLease {
         pool->cv.notify_one();
     }
     char *mem() const { return pool->mem + (size_t)id * pool->block_bytes; }
+    char *staging() const { return pool->staging + (size_t)id * pool->staging_bytes; }
     cudaStream_t stream() const { return pool->streams[id]; }
 };
 
@@ -1129,6 +1137,24 @@ extern "C" int fann_pool_create(fann_index *ix, uint32_t n_blocks, uint32_t max_
         p->streams.push_back(st);
         p->free_blocks.push_back(n_blocks - 1 - i);
     }
+    p->graphs.resize(n_blocks);
+    if (const char *sg = getenv("FANN_SMALL_GRAPH")) p->use_graphs = atoi(sg) != 0;
+    if (max_nprobe && p->use_graphs) {                         // staging for the graph replays of the posting-list form
+        size_t o = 0;
+        p->st_queries = o; o = align_up(o + (size_t)max_B * ix->M * dsub * 4, 256);
+        p->st_probes = o;  o = align_up(o + (size_t)max_B * max_nprobe * 4, 256);
+        p->st_ids = o;     o = align_up(o + (size_t)max_B * k_max * 4, 256);
+        p->st_dists = o;   o = align_up(o + (size_t)max_B * k_max * 4, 256);
+        p->st_counts = o;  o = align_up(o + (size_t)max_B * 4, 256);
+        p->st_hdr = o;     o = align_up(o + sizeof(ListsHeader) + sizeof(WsHeader), 256);
+        p->staging_bytes = o;
+        if (cudaHostAlloc(&p->staging, o * n_blocks, cudaHostAllocDefault) != cudaSuccess) {
+            p->staging = nullptr; p->use_graphs = false;       // no pinned memory: plain launches
+            cudaGetLastError();
+        }
+    } else {
+        p->use_graphs = false;
+    }
     *out = p;
     return FANN_OK;
 }
@@ -1138,6 +1164,8 @@ extern "C" void fann_pool_destroy(fann_pool *p)
     if (!p) return;
     DeviceGuard guard(p->ix->device);
     for (auto st : p->streams) { cudaStreamSynchronize(st); cudaStreamDestroy(st); }
+    for (auto &blk : p->graphs) for (auto &g : blk) cudaGraphExecDestroy(g.exec);
+    if (p->staging) cudaFreeHost(p->staging);
     if (p->mem) cudaFree(p->mem);
     delete p;
 }
@@ -1177,8 +1205,66 @@ extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const fl
         return fail(FANN_EINVAL, "fann_search_small_lists: B=%u (pool: %u), k=%u (pool: %u), dsub=%u (pool: %u), nprobe=%u (pool: %u)",
                     B, pool->max_B, k, pool->k_max, dsub, pool->dsub, nprobe, pool->max_nprobe);
     BlockLease lease(pool);
-    return fann_search_lists_host(ix, queries_h, B, codebooks_d, dsub, probes_h, nprobe, pool->max_cands, k, out_ids_h,
-                                  out_dists_h, out_counts_h, lease.mem(), pool->block_bytes, lease.stream());
+    if (!pool->use_graphs)
+        return fann_search_lists_host(ix, queries_h, B, codebooks_d, dsub, probes_h, nprobe, pool->max_cands, k, out_ids_h,
+                                      out_dists_h, out_counts_h, lease.mem(), pool->block_bytes, lease.stream());
+    // One cudaGraphLaunch per call: the block's graph for this call shape copies queries and probes up from the
+    // block's pinned staging buffer, runs the path and copies results and the two status headers back.
+    if (!queries_h || !codebooks_d || !probes_h || !out_ids_h || !out_dists_h)
+        return fail(FANN_EINVAL, "fann_search_small_lists: NULL argument");
+    if (!ix->codes || !ix->list_offsets) return fail(FANN_EINVAL, "fann_search_small_lists: load codes and posting lists first");
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = lease.stream();
+    char *st = lease.staging(), *s = lease.mem();
+    const size_t qbytes = (size_t)B * ix->M * dsub * 4, pbytes = (size_t)B * nprobe * 4, obytes = (size_t)B * k * 4;
+    memcpy(st + pool->st_queries, queries_h, qbytes);
+    memcpy(st + pool->st_probes, probes_h, pbytes);
+    ListsHostScratch h;
+    lists_host_layout(ix, B, dsub, nprobe, pool->max_cands, k, &h);
+    ListsLayout l;
+    lists_layout(ix, B, pool->max_cands, k, &l);
+    cudaGraphExec_t exec = nullptr;
+    for (auto &g : pool->graphs[lease.id])
+        if (g.B == B && g.nprobe == nprobe && g.k == k && g.codebooks == codebooks_d) exec = g.exec;
+    if (!exec) {
+        CUDA_TRY(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
+        int rc = FANN_OK;
+        cudaError_t ce = cudaMemcpyAsync(s + h.queries, st + pool->st_queries, qbytes, cudaMemcpyHostToDevice, stream);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(s + h.probes, st + pool->st_probes, pbytes, cudaMemcpyHostToDevice, stream);
+        if (ce == cudaSuccess) rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
+        if (ce == cudaSuccess && rc == FANN_OK)
+            rc = search_lists_impl(ix, (const float *)(s + h.lut), B, (const uint32_t *)(s + h.probes), nprobe, pool->max_cands, k,
+                                   (uint32_t *)(s + h.out_ids), (float *)(s + h.out_dists), (uint32_t *)(s + h.out_counts), nullptr,
+                                   s + h.ws, l, stream);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_ids, s + h.out_ids, obytes, cudaMemcpyDeviceToHost, stream);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_dists, s + h.out_dists, obytes, cudaMemcpyDeviceToHost, stream);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_counts, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_hdr, s + h.ws + l.hdr, sizeof(ListsHeader), cudaMemcpyDeviceToHost, stream);
+        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_hdr + sizeof(ListsHeader), s + h.ws + l.ws, sizeof(WsHeader), cudaMemcpyDeviceToHost, stream);
+        cudaGraph_t graph = nullptr;
+        cudaError_t ee = cudaStreamEndCapture(stream, &graph);
+        if (rc != FANN_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (ce != cudaSuccess || ee != cudaSuccess || !graph) {
+            if (graph) cudaGraphDestroy(graph);
+            return fail(FANN_ECUDA, "fann_search_small_lists: graph capture: %s", cudaGetErrorString(ce != cudaSuccess ? ce : ee));
+        }
+        ce = cudaGraphInstantiate(&exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (ce != cudaSuccess) return fail(FANN_ECUDA, "fann_search_small_lists: cudaGraphInstantiate: %s", cudaGetErrorString(ce));
+        pool->graphs[lease.id].push_back({B, nprobe, k, codebooks_d, exec});
+    }
+    CUDA_TRY(cudaGraphLaunch(exec, stream));
+    CUDA_TRY(cudaStreamSynchronize(stream));
+    const ListsHeader *lh = (const ListsHeader *)(st + pool->st_hdr);
+    const WsHeader *wh = (const WsHeader *)(st + pool->st_hdr + sizeof(ListsHeader));
+    if (lh->overflow)
+        return fail(FANN_EWORKSPACE, "the probed lists hold %llu candidate IDs, the pool's blocks hold %llu", lh->total, lh->capacity);
+    if (wh->status & kStatusPlanOverflow) return fail(FANN_EINVAL, "total_cands passed to the call was smaller than cand_offsets[B]");
+    if (wh->status & kStatusTableFull) return fail(FANN_EOVERFLOW, "a dedup hash table filled up (colliding candidate IDs)");
+    memcpy(out_ids_h, st + pool->st_ids, obytes);
+    memcpy(out_dists_h, st + pool->st_dists, obytes);
+    if (out_counts_h) memcpy(out_counts_h, st + pool->st_counts, (size_t)B * 4);
+    return FANN_OK;
 }
 
 // ---------------------------------------------------------------- NEXT-1: heuristic re-ranking

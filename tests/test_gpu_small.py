@@ -110,7 +110,11 @@ def _pool(fann, ix, w, n_blocks, max_B):
     return fann.fann_pool_create(ix.handle, n_blocks, max_B, per_q * max_B, w.cfg.dsub, w.cfg.nprobe, w.cfg.k)
 
 
-def test_pool_entries_match_the_oracle(fann, wl, ref):
+@pytest.mark.parametrize("graphs", ["1", "0"])
+def test_pool_entries_match_the_oracle(fann, wl, ref, monkeypatch, graphs):
+    """Both entry forms on a pool block; the posting-list form replays one CUDA graph per call shape
+    (FANN_SMALL_GRAPH=0: plain launches) -- the second call of a shape is a pure replay."""
+    monkeypatch.setenv("FANN_SMALL_GRAPH", graphs)
     w = wl
     ix = fann.FannIndex(0)
     ix.load_codes(w.codes.to(DEV))
@@ -118,7 +122,7 @@ def test_pool_entries_match_the_oracle(fann, wl, ref):
     pool = _pool(fann, ix, w, 2, 4)
     cb = w.codebooks.to(DEV)
     k = w.cfg.k
-    for b0, b1 in ((0, 1), (1, 4), (4, 8), (39, 40)):
+    for b0, b1 in ((0, 1), (1, 4), (4, 8), (39, 40), (7, 8), (20, 23)):
         B = b1 - b0
         q, off, ids = _sub(w, b0, b1)
         for form in ("ids", "lists"):
@@ -133,7 +137,7 @@ def test_pool_entries_match_the_oracle(fann, wl, ref):
             assert np.array_equal(oi, r["ids"]) and np.array_equal(od.view(np.uint32), r["dists"].view(np.uint32))
             assert np.array_equal(oc, r["counts"])
     st = fann.fann_pool_stats(pool)
-    assert st["calls"] == 8 and st["in_use"] == 0 and st["n_blocks"] == 2 and st["high_water"] == 1
+    assert st["calls"] == 12 and st["in_use"] == 0 and st["n_blocks"] == 2 and st["high_water"] == 1
     # what the pool was not created for
     q, off, ids = _sub(w, 0, 5)
     oi, od, oc = np.zeros((5, k), np.uint32), np.zeros((5, k), np.float32), np.zeros(5, np.uint32)
