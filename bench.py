@@ -367,6 +367,7 @@ def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=F
     barrier()
     t1 = time.time()
     fann.fann_workspace_status(ix.handle, ws, stream)               # raises if any timed step overflowed a table
+    modes = fann.fann_workspace_modes(ix.handle, ws, B, total, k, stream)
     launches = ix.info()["kernel_launches"] - launches0
     fann.fann_set_timing(ix.handle, False)
     total_ms = float(sum(a.elapsed_time(b) for a, b in ev))
@@ -389,7 +390,8 @@ def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=F
                 "code_bytes_only_frac": round(M * U_total / (scan_ms * 1e-3) / 1e9 / peak, 4),
                 "rows_per_s": U_total / (scan_ms * 1e-3),
                 "share_of_step": round(scan_ms / ms_per_step, 4),
-                "kernels_ms": {kk: round(float(np.mean(v)), 4) for kk, v in kern.items()}}
+                "kernels_ms": {kk: round(float(np.mean(v)), 4) for kk, v in kern.items()},
+                "dedup_placement": modes}
     res = {"ms_per_step": ms_per_step, "value": U_all / (ms_per_step * 1e-3), "U_all": U_all, "C_all": C_all,
            "U_total": U_total, "C_total": total, "roofline": roofline, "launches": int(launches), "clocks": clocks,
            "path_algorithmic_bytes": path_bytes, "path_hbm_frac": round(path_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4),

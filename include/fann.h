@@ -169,6 +169,14 @@ int fann_dedup_only(fann_index *ix, uint32_t B, const int64_t *cand_offsets,
 int fann_workspace_status(fann_index *ix, const void *workspace, void *stream);
 
 /*
+ * Diagnostics: how many queries of the last fann_dedup_scan_topk / fann_dedup_only call on this
+ * workspace (same B, total_cands, k) were deduplicated with order-preserving placement and how
+ * many fell back to hashed placement (bunched IDs).  Synchronises `stream`.
+ */
+int fann_workspace_modes(fann_index *ix, const void *workspace, uint32_t B, uint64_t total_cands, uint32_t k,
+                         uint32_t *n_ordered, uint32_t *n_hashed, void *stream);
+
+/*
  * The whole stage from HOST buffers, for callers that hold the batch in host
  * memory (the paper's step (4): the CPU sends the vector-IDs):
  * copies queries / candidate lists host->device into `device_scratch`, runs

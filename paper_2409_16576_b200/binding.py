@@ -71,6 +71,7 @@ def load_library():
         "fann_dedup_scan_topk": (i, [p, p, u32, p, p, u64, u32, p, p, p, p, p, sz, p]),
         "fann_dedup_only": (i, [p, u32, p, p, u64, p, p, p, sz, p]),
         "fann_workspace_status": (i, [p, p, p]),
+        "fann_workspace_modes": (i, [p, p, u32, u64, u32, C.POINTER(u32), C.POINTER(u32), p]),
         "fann_search_host_scratch_bytes": (sz, [p, u32, u32, u64, u32]),
         "fann_search_host": (i, [p, p, u32, p, u32, p, p, u32, p, p, p, p, sz, p]),
         "fann_load_lists": (i, [p, p, p, u64, u64, i, p]),
@@ -325,6 +326,12 @@ def fann_get_info(ix) -> dict:
 
 def fann_set_timing(ix, enable: bool) -> None:
     _check(load_library().fann_set_timing(ix, int(enable)))
+
+
+def fann_workspace_modes(ix, workspace, B, total_cands, k, stream=None) -> dict:
+    a, b = C.c_uint32(0), C.c_uint32(0)
+    _check(load_library().fann_workspace_modes(ix, _addr(workspace), B, total_cands, k, C.byref(a), C.byref(b), stream))
+    return {"ordered": int(a.value), "hashed": int(b.value)}
 
 
 def fann_last_timing(ix) -> dict:

@@ -639,6 +639,26 @@ extern "C" int fann_workspace_status(fann_index *ix, const void *workspace, void
     return FANN_OK;
 }
 
+extern "C" int fann_workspace_modes(fann_index *ix, const void *workspace, uint32_t B, uint64_t total_cands, uint32_t k,
+                                    uint32_t *n_ordered, uint32_t *n_hashed, void *stream)
+{
+    if (!ix || !workspace || B == 0) return fail(FANN_EINVAL, "fann_workspace_modes: bad argument");
+    if (!ix->codes || k == 0 || k > FANN_MAX_K) return fail(FANN_EINVAL, "fann_workspace_modes: bad argument");
+    DeviceGuard guard(ix->device);
+    Geom g;
+    geometry(ix, k, B, total_cands, &g);
+    WsLayout w;
+    ws_layout(B, total_cands, g, true, &w);
+    std::vector<uint32_t> mode(B);
+    CUDA_TRY(cudaMemcpyAsync(mode.data(), (const char *)workspace + w.mode, (size_t)B * 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    uint32_t h = 0;
+    for (uint32_t b = 0; b < B; ++b) h += mode[b] == kModeHashed ? 1u : 0u;
+    if (n_ordered) *n_ordered = B - h;
+    if (n_hashed) *n_hashed = h;
+    return FANN_OK;
+}
+
 // ---------------------------------------------------------------- host-buffer entry
 
 struct HostScratch {
