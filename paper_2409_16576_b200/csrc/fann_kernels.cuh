@@ -7,13 +7,16 @@
 //   mode_kernel          per query: order-preserving or hashed placement in the dedup table
 //   partition_kernel     split each query's candidate IDs into its S_b classes (ID ranges or hash
 //                        classes), so that each dedup pass reads only its own IDs
-//   dedup_kernel<T>      (5) shared-memory dedup table, one (query, partition) per CTA pass; probe /
-//                        store / verify phases separated by barriers, no atomics in the table;
-//                        writes the distinct IDs of every query as a compact list, ascending in
-//                        ordered mode (up to the compaction step and probe displacement)
-//   scan_kernel<G,NB,D>  (6) code-row gather through a per-warp shared-memory ring filled by
+//   partition_multi_kernel  the same with several CTAs per query (small batches)
+//   dedup_kernel<T,R>    (5) shared-memory dedup table of 16-byte buckets, one (query, partition) per CTA
+//                        pass; straight-line read / write / verify rounds separated by barriers, no
+//                        atomics in the table; writes the distinct IDs of every query as a compact
+//                        list, ascending in ordered mode (up to a bucket and overflow displacement)
+//   scan_kernel<G,NB,D,LM>  (6) code-row gather through a per-warp shared-memory ring filled by
 //                        asynchronous copies + Eq. 1 ADC from a conflict-free table  (7) streaming
-//                        top-k, one query per CTA pass; writes out_ids / out_dists / counts
+//                        top-k, one query (or one slice of its distinct list) per CTA pass; writes
+//                        out_ids / out_dists / counts.  LM: the list-major experiment
+//   merge_parts_kernel   (7) small batches: merges the partial top-k of a query's scan CTAs
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -23,7 +26,6 @@ namespace fann {
 constexpr uint32_t kIdNone = 0xFFFFFFFFu;
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;             // empty hash slot (never a valid id: id < N < 2^32-1)
 constexpr unsigned long long kKeyMax = ~0ull;        // padding key, sorts last
-constexpr int kDedupThreads = 1024;
 constexpr int kScanThreads = 512;
 constexpr int kScanWarps = kScanThreads / 32;
 constexpr int kSample = 256;                         // keys sampled to place a prune pivot
