@@ -219,6 +219,17 @@ def gather_ceiling(fann, ix, w, dev, nq_groups: int = 4):
             "shuffled_cp_async_ring": rate(rnd, 3)}
 
 
+def same_ids(cfg, a, b) -> bool:
+    """Two runs of the path on one batch: the same bytes on integer data; on real-valued data a row's fp32 sum depends
+    on the lane that scores it, so neighbours a rounding apart may swap places (tolerance regime): the
+    runs must agree on at least 99.9 % of the output slots."""
+    import numpy as np
+    a, b = np.asarray(a).view(np.int32), np.asarray(b).view(np.int32)
+    if cfg.integer_exact:
+        return bool(np.array_equal(a, b))
+    return bool(a.shape == b.shape and np.mean(a == b) >= 0.999)
+
+
 def _probe_lib():
     import ctypes as C
     from paper_2409_16576_b200.build import build_probe
@@ -424,7 +435,7 @@ def small_batch_leg(fann, ix, w, cfg, dev, ref_ids):
             t0 = time.perf_counter()
             fann.fann_search_small_lists(ix.handle, pool, q_h[b0:b0 + B], B, w.codebooks, dsub, p_h[b0:b0 + B], nprobe, k, oi, od, oc)
             ts.append(time.perf_counter() - t0)
-            ok = ok and bool(np.array_equal(oi.view(np.int32), ref_ids[b0:b0 + B]))
+            ok = ok and same_ids(cfg, oi, ref_ids[b0:b0 + B])
         ts = sorted(ts[4:])
         res[f"B{B}"] = {"latency_us_p50": round(1e6 * ts[len(ts) // 2], 1), "latency_us_p90": round(1e6 * ts[int(len(ts) * 0.9)], 1),
                         "qps_one_thread": round(B / ts[len(ts) // 2], 1)}
@@ -501,7 +512,7 @@ def list_major_leg(fann, ix, w, cfg, args, dev, ref_ids, U_total, C_total):
             "ms_per_step": round(ms, 4), "value": U_total / (ms * 1e-3), "unit": UNIT,
             "rows_scored_per_s": C_total / (ms * 1e-3), "extra_hbm_bytes": need_copy, "build_ms": round(build_ms, 1),
             "algorithmic_bytes": bytes_, "hbm_frac": round(bytes_ / (ms * 1e-3) / 1e9 / peak, 4),
-            "matches_device_path": bool(np.array_equal(oi.cpu().numpy(), ref_ids))}
+            "matches_device_path": same_ids(cfg, oi.cpu().numpy(), ref_ids)}
 
 
 def sample_parity(w, cfg, out, nq):
@@ -646,7 +657,7 @@ def main():
         e2e = {"value": U_total / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": round(e_ms, 3),
                "entry": "fann_search_lists_host (posting lists resident in HBM, PAPER.md:L125 step 3 on the GPU)",
                "h2d_bytes_per_step": int(q_h.numel() * 4 + p_h.numel() * 4), "d2h_bytes_per_step": d2h,
-               "matches_device_path": bool(np.array_equal(oi.numpy(), ref_ids))}
+               "matches_device_path": same_ids(cfg, oi.numpy(), ref_ids)}
         del scratch, p_h
         torch.cuda.empty_cache()
         try:
@@ -667,7 +678,7 @@ def main():
         e2e_ids = {"value": U_total / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": round(e_ms, 3),
                    "entry": "fann_search_host (candidate IDs from the host, PAPER.md:L125 step 4)",
                    "h2d_bytes_per_step": int(q_h.numel() * 4 + off_h.numel() * 8 + ids_h.numel() * 4),
-                   "d2h_bytes_per_step": d2h, "matches_device_path": bool(np.array_equal(oi.numpy(), ref_ids))}
+                   "d2h_bytes_per_step": d2h, "matches_device_path": same_ids(cfg, oi.numpy(), ref_ids)}
         del scratch, q_h, ids_h, off_h
 
     ms_per_step = res["ms_per_step"]
