@@ -215,6 +215,11 @@ int fann_search_host(fann_index *ix, const float *queries_h, uint32_t B,
  * list_offsets  [n_lists + 1] int64, list_offsets[0] == 0, list_offsets[n_lists] == n_entries
  * list_ids      [n_entries] uint32 vector-IDs (any order inside a list)
  * Host or device source (src_is_device); synchronises `stream`.
+ * If the codes are loaded already (N is known) the library sorts every list of its copy
+ * ascending and indexes it by 64 ID-range cells (130 bytes per list more): fann_search_lists
+ * then takes every dedup partition's IDs straight from the probed lists and writes neither a
+ * candidate array nor its split (nprobe <= 512; lists longer than 8192 entries, lists loaded
+ * before the codes, or FANN_LISTS_DIRECT=0 take the expanding path).  Same results either way.
  * Errors: EINVAL (NULL, n_lists == 0, offsets do not end at n_entries), ENOMEM, ECUDA.
  */
 int fann_load_lists(fann_index *ix, const int64_t *list_offsets, const uint32_t *list_ids,

@@ -39,6 +39,9 @@ struct fann_index {
     uint64_t vec_N = 0;
     uint32_t vec_d = 0;
     int vec_elem = 0;
+    uint16_t *list_grid = nullptr;         // [n_lists][kGridCells + 1]: sorted lists' positions of the ID-range cells
+    bool lists_sorted = false;             // every list was sorted and indexed at load (lists-direct path possible)
+    bool lists_direct = true;              // FANN_LISTS_DIRECT=0: always expand + split (the path of unsorted lists)
     uint8_t *lm_codes = nullptr;           // list-major experiment: [list_entries][row_bytes], row e = code of list_ids[e]
     uint32_t *page_of = nullptr;           // [page_N]
     uint64_t page_N = 0, n_pages = 0;
@@ -142,17 +145,18 @@ struct Geom {
 // list needs two or more partitions anyway -- two 512-thread CTAs per SM with half the table each, so that one computes
 // while the other waits at a barrier (partition_kernel makes the number of partitions free: each ID is read once).
 static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t total_cands, Geom *g, uint32_t shape = 0,
-                     bool allow_split = true)
+                     bool allow_split = true, bool ld = false)
 {
+    const uint32_t ldb = ld ? dedup_ld_bytes() : 0u;           // lists-direct: the segment table sits before the dedup table
     g->dedup_threads = 1024; g->dedup_smem = ix->dedup_smem;
-    g->nslots_max = ((g->dedup_smem - dedup_table_off(1024)) / 4) & ~3u;
+    g->nslots_max = ((g->dedup_smem - dedup_table_off(1024) - ldb) / 4) & ~3u;
     g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);      // <= 75 % load even with no repeats
     const uint64_t mean_c = total_cands / (B ? B : 1);
     const bool split = shape ? shape == 512
-                             : (ix->dedup_threads == 512 || (ix->dedup_threads == 0 && ix->partition && mean_c > g->cap_c));
+                             : (ix->dedup_threads == 512 || (ix->dedup_threads == 0 && (ix->partition || ld) && mean_c > g->cap_c));
     if (split && ix->dedup_smem_half >= 32768) {
         g->dedup_threads = 512; g->dedup_smem = ix->dedup_smem_half;
-        g->nslots_max = ((g->dedup_smem - dedup_table_off(512)) / 4) & ~3u;
+        g->nslots_max = ((g->dedup_smem - dedup_table_off(512) - ldb) / 4) & ~3u;
         g->cap_c = (uint32_t)((uint64_t)g->nslots_max * 3 / 4);
     }
     g->ring = ix->scan_ring;
@@ -178,7 +182,7 @@ struct WsLayout {
 
 static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with_uniq, WsLayout *w)
 {
-    const uint64_t max_items = (uint64_t)B + total_cands / g.cap_c + 1;
+    const uint64_t max_items = 2 * ((uint64_t)B + total_cands / g.cap_c + 1);   // x2: the lists-direct path rounds S_b up to a power of two
     w->max_items = (uint32_t)(max_items > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : max_items);
     size_t o = 0;
     w->hdr = o;         o = align_up(o + 256, 256);
@@ -227,6 +231,8 @@ extern "C" int fann_create(fann_index **out, int device)
                     smem_optin, scan_max);
     CUDA_TRY((cudaFuncSetAttribute(dedup_kernel<1024, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)));
     CUDA_TRY((cudaFuncSetAttribute(dedup_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)));
+    CUDA_TRY((cudaFuncSetAttribute(dedup_kernel<1024, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)));
+    CUDA_TRY((cudaFuncSetAttribute(dedup_kernel<512, 8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)));
     const int ring_max = (int)scan_smem_bytes(4096, 3);
     if (ring_max > smem_optin)
         return fail(FANN_EUNSUPPORTED, "fann_create: device offers %d bytes of shared memory per block, %d needed",
@@ -253,6 +259,7 @@ extern "C" int fann_create(fann_index **out, int device)
     if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
     if (const char *s = getenv("FANN_PARTITION")) ix->partition = atoi(s) != 0;
     if (const char *s = getenv("FANN_SPLIT_SCAN")) ix->split_scan = atoi(s) != 0;
+    if (const char *s = getenv("FANN_LISTS_DIRECT")) ix->lists_direct = atoi(s) != 0;
     if (const char *s = getenv("FANN_SCAN_RING")) { int v = atoi(s); if (v == 0 || v == 3) ix->scan_ring = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_THREADS")) { int v = atoi(s); if (v == 512 || v == 1024) ix->dedup_threads = (uint32_t)v; }
     *out = ix;
@@ -271,6 +278,7 @@ extern "C" void fann_destroy(fann_index *ix)
     if (ix->vectors) cudaFree(ix->vectors);
     if (ix->page_of) cudaFree(ix->page_of);
     if (ix->lm_codes) cudaFree(ix->lm_codes);
+    if (ix->list_grid) cudaFree(ix->list_grid);
     for (CallCtx *c : ix->ctx_pool) destroy_ctx(c);
     for (auto &e : ix->ev_lut) if (e) cudaEventDestroy(e);
     for (auto &e : ix->ev_plan) if (e) cudaEventDestroy(e);
@@ -457,10 +465,14 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                     uint32_t k, uint32_t *out_ids, float *out_dists, uint32_t *out_counts,
                     uint32_t *out_uniq, uint32_t *uniq_ids, uint32_t *uniq_counts,
                     void *workspace, size_t workspace_bytes, cudaStream_t stream,
-                    uint32_t shape = 0, bool keep_status = false, bool exact_total = true, bool allow_split = true)
+                    uint32_t shape = 0, bool keep_status = false, bool exact_total = true, bool allow_split = true,
+                    const uint32_t *probes = nullptr, uint32_t nprobe = 0)
 {
+    // probes != NULL: lists-direct (fann_search_lists on sorted posting lists): cand_ids is not read, the dedup kernel
+    // takes every item's IDs straight from the probed lists
+    const bool ld = probes != nullptr;
     Geom g;
-    geometry(ix, k, B, total_cands, &g, shape, allow_split);
+    geometry(ix, k, B, total_cands, &g, shape, allow_split, ld);
     WsLayout w;
     ws_layout(B, total_cands, g, !dump, &w);
     if (!workspace || ((uintptr_t)workspace & 255) != 0)
@@ -488,15 +500,20 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     plan_kernel<<<1, 1024, 0, stream>>>((const long long *)cand_offsets, B, g.cap_c, w.max_items, hdr, S,
                                         item_start, items, uniq_counts, keep_status ? 1u : 0u,
                                         (unsigned long long)total_cands, exact_total ? 1u : 0u,
-                                        g.part_ctas > 1 ? (uint32_t *)(ws + w.bucket_cnt) : nullptr,
-                                        g.part_ctas > 1 ? (uint32_t *)(ws + w.part_aux) : nullptr);
-    mode_kernel<<<(B + 7) / 8, 256, 0, stream>>>((const long long *)cand_offsets, cand_ids, B, ix->N,
-                                                  ix->force_mode, ix->partition ? 0u : g.cap_c, mode);
+                                        g.part_ctas > 1 && !ld ? (uint32_t *)(ws + w.bucket_cnt) : nullptr,
+                                        g.part_ctas > 1 && !ld ? (uint32_t *)(ws + w.part_aux) : nullptr, ld ? 1u : 0u);
+    if (ld)
+        lists_classes_kernel<<<B, 256, 0, stream>>>(ix->list_grid, ix->n_lists, ix->N, probes, nprobe, S, item_start,
+                                                    (uint32_t)((uint64_t)g.nslots_max * 9 / 10), ix->force_mode, mode,
+                                                    (uint32_t *)(ws + w.bucket_cnt));
+    else
+        mode_kernel<<<(B + 7) / 8, 256, 0, stream>>>((const long long *)cand_offsets, cand_ids, B, ix->N,
+                                                      ix->force_mode, ix->partition ? 0u : g.cap_c, mode);
     if (timing) cudaEventRecord(ix->ev_plan[1], stream);
     ix->launches += 2;
     CUDA_TRY(cudaGetLastError());
 
-    uint32_t chunks = dump ? 1u : ix->chunks;
+    uint32_t chunks = (dump || ld) ? 1u : ix->chunks;
     if (chunks > B) chunks = B;
     const bool overlap = chunks > 1 && ix->partition;
     CtxLease lease(overlap ? ix : nullptr);                    // returned to the pool when the call returns
@@ -513,6 +530,8 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     dp.uniq_ids = uniq_ids; dp.uniq_counts = uniq_counts;
     dp.part_ids = ix->partition ? (const uint32_t *)(ws + w.part_ids) : nullptr;
     dp.part_ok = (const uint32_t *)(ws + w.part_ok); dp.bucket_cnt = (const uint32_t *)(ws + w.bucket_cnt);
+    dp.list_offsets = ix->list_offsets; dp.list_ids = ix->list_ids; dp.list_grid = ix->list_grid;
+    dp.probes = probes; dp.nprobe = nprobe; dp.n_lists = ix->n_lists;
     PartParams pp;
     pp.cand_offsets = (const long long *)cand_offsets; pp.cand_ids = cand_ids; pp.N = ix->N;
     pp.S = S; pp.mode = mode; pp.item_start = item_start;
@@ -547,7 +566,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
     for (uint32_t c = 0; c < chunks; ++c) {
         const uint32_t qb = (uint32_t)((uint64_t)B * c / chunks), qe = (uint32_t)((uint64_t)B * (c + 1) / chunks);
         if (overlap) CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_done[c], 0));
-        if (!overlap && ix->partition && c == 0) {
+        if (!overlap && ix->partition && c == 0 && !ld) {
             pp.q_begin = 0;
             if (timing) cudaEventRecord(ix->ev_part[0], stream);
             if (g.part_ctas > 1) partition_multi_kernel<<<B * g.part_ctas, kPartThreads, 0, stream>>>(pp);
@@ -558,7 +577,10 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
         }
         if (timing) cudaEventRecord(ix->ev_dedup[c][0], stream);
         dp.q_begin = qb; dp.q_end = qe; dp.counter = &hdr->dedup_counter[c];
-        if (g.dedup_threads == 512) dedup_kernel<512, 8><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
+        if (ld) {
+            if (g.dedup_threads == 512) dedup_kernel<512, 8, true><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
+            else dedup_kernel<1024, 8, true><<<ix->num_sms, 1024, g.dedup_smem, stream>>>(dp);
+        } else if (g.dedup_threads == 512) dedup_kernel<512, 8><<<2 * ix->num_sms, 512, g.dedup_smem, stream>>>(dp);
         else dedup_kernel<1024, 8><<<ix->num_sms, 1024, g.dedup_smem, stream>>>(dp);
         if (timing) cudaEventRecord(ix->ev_dedup[c][1], stream);
         ix->launches++;
@@ -791,15 +813,44 @@ extern "C" int fann_load_lists(fann_index *ix, const int64_t *list_offsets, cons
                     ends[0], ends[1], (unsigned long long)n_entries);
     }
     ix->n_lists = n_lists; ix->list_entries = n_entries;
+    // Sort every list and index it by ID-range cell (needs N: load the codes first), so that fann_search_lists can
+    // read a class's IDs straight from the lists.  The order of a list's IDs carries no meaning (L150).
+    ix->lists_sorted = false;
+    if (ix->list_grid) { cudaFree(ix->list_grid); ix->list_grid = nullptr; }
+    if (ix->codes && ix->N && n_entries < 0xFFFFFFFFull) {
+        uint32_t *flag = nullptr;
+        if (cudaMalloc(&ix->list_grid, n_lists * (kGridCells + 1) * sizeof(uint16_t)) == cudaSuccess &&
+            cudaMalloc(&flag, 4) == cudaSuccess) {
+            CUDA_TRY(cudaMemsetAsync(flag, 0, 4, stream));
+            lists_sort_grid_kernel<<<(unsigned)n_lists, 256, kSortMaxList * 4, stream>>>(ix->list_offsets, ix->list_ids, ix->N,
+                                                                                       ix->list_grid, flag);
+            ix->launches++;
+            uint32_t unsorted = 1;
+            cudaError_t e2 = cudaMemcpyAsync(&unsorted, flag, 4, cudaMemcpyDeviceToHost, stream);
+            if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(stream);
+            cudaFree(flag);
+            if (e2 != cudaSuccess) return fail(FANN_ECUDA, "fann_load_lists: sorting the lists: %s", cudaGetErrorString(e2));
+            ix->lists_sorted = unsorted == 0;
+        } else {
+            if (ix->list_grid) { cudaFree(ix->list_grid); ix->list_grid = nullptr; }
+            if (flag) cudaFree(flag);
+            cudaGetLastError();
+        }
+    }
     return FANN_OK;
 }
 
 struct ListsLayout { size_t hdr, offsets, ids, ws, ws_bytes, total; };
 
+static bool lists_direct_ok(const fann_index *ix, uint32_t nprobe)
+{
+    return ix->lists_direct && ix->lists_sorted && ix->list_grid && nprobe <= kLdMaxProbe;
+}
+
 static void lists_layout(const fann_index *ix, uint32_t B, uint64_t cap, uint32_t k, ListsLayout *l)
 {
     Geom g;
-    geometry(ix, k, B, cap, &g);
+    geometry(ix, k, B, cap, &g, 0, true, ix->lists_direct && ix->lists_sorted);   // the direct path's tables are a little smaller
     WsLayout w;
     ws_layout(B, cap, g, true, &w);
     size_t o = 0;
@@ -832,6 +883,14 @@ static int search_lists_impl(fann_index *ix, const float *lut, uint32_t B, const
                                                          (unsigned long long *)offsets);
     lists_scan_kernel<<<1, 1024, 0, stream>>>((const unsigned long long *)offsets, B, offsets, hdr,
                                               (unsigned long long)max_total_cands);
+    if (lists_direct_ok(ix, nprobe)) {
+        // sorted lists with a grid: no candidate array, no class split -- the dedup kernel reads every class's IDs
+        // straight from the probed lists (cand_offsets only places the queries' distinct lists)
+        ix->launches += 2;
+        CUDA_TRY(cudaGetLastError());
+        return run_path(ix, false, lut, B, (const int64_t *)offsets, ids, max_total_cands, k, out_ids, out_dists, out_counts,
+                        out_uniq, nullptr, nullptr, ws + l.ws, l.ws_bytes, stream, 0, false, false, true, probes, nprobe);
+    }
     uint32_t expand_ctas = 1;                                  // small batches: spread a query's lists over several CTAs
     while (expand_ctas < 16 && 2 * expand_ctas * B <= (uint32_t)ix->num_sms && 8 * expand_ctas < nprobe) expand_ctas <<= 1;
     lists_expand_kernel<<<B * expand_ctas, kExpandThreads, ((size_t)nprobe + 1) * 4, stream>>>(

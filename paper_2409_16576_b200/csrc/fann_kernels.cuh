@@ -30,6 +30,7 @@ constexpr int kScanThreads = 512;
 constexpr int kScanWarps = kScanThreads / 32;
 constexpr int kSample = 256;                         // keys sampled to place a prune pivot
 constexpr int kMaxChunks = 16;                       // batch chunks (dedup of chunk i+1 overlaps scan of chunk i)
+constexpr uint32_t kGridCells = 64;                  // ID-range cells sorted posting lists are indexed by (lists-direct: S | 64)
 constexpr uint32_t kStatusTableFull = 1u;
 constexpr uint32_t kStatusPlanOverflow = 2u;
 
@@ -191,7 +192,8 @@ __global__ void __launch_bounds__(256) build_lut_kernel(const float *__restrict_
 __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t B, uint32_t cap_c,
                             uint32_t max_items, WsHeader *hdr, uint32_t *S, uint32_t *item_start,
                             uint2 *items, uint32_t *uniq_counts, uint32_t keep_status,
-                            unsigned long long total_cands, uint32_t exact_total, uint32_t *bucket_cnt, uint32_t *part_aux)
+                            unsigned long long total_cands, uint32_t exact_total, uint32_t *bucket_cnt, uint32_t *part_aux,
+                            uint32_t pow2_classes)
 {
     __shared__ uint32_t warp_sums[32];
     __shared__ uint32_t running;
@@ -214,6 +216,11 @@ __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t
             if (c < 0) c = 0;
             s = (uint32_t)((c + cap_c - 1) / cap_c);
             if (s == 0) s = 1;
+            if (pow2_classes && s <= kGridCells) {             // lists-direct: ID-range classes are runs of grid cells
+                uint32_t s2 = 1;
+                while (s2 < s) s2 <<= 1;
+                s = s2;
+            }
             if (refuse) s = 0;                                 // no partition, no dedup item; the scan sees U = 0
             S[b] = s;
             uniq_counts[b] = 0;
@@ -335,7 +342,22 @@ struct DedupParams {
     const uint32_t *part_ids;                        // [2 * total_cands] buckets written by partition_kernel, or NULL
     const uint32_t *part_ok;                         // [B] 1: query b's buckets are valid
     const uint32_t *bucket_cnt;                      // [n_items] IDs in the bucket of each (query, partition) item
+    // Lists-direct mode (dedup_kernel<..., LD = true>, fann_search_lists on sorted posting lists): the IDs of an item
+    // are read straight from the probed lists -- for an ID-range class the sub-range of every list that falls into
+    // it, found in the lists' grid -- so that neither a candidate array nor its class split is ever written.
+    const long long *list_offsets;                   // [n_lists + 1]
+    const uint32_t *list_ids;                        // every list ascending
+    const uint16_t *list_grid;                       // [n_lists][kGridCells + 1] position of the first ID >= cell start
+    const uint32_t *probes;                          // [B][nprobe]
+    uint32_t nprobe;
+    uint64_t n_lists;
 };
+
+constexpr uint32_t kLdMaxProbe = 512;                // lists-direct: probes per query the shared-memory segment table holds
+constexpr uint32_t kLdRowMap = 1024;                 // lists-direct: 32-ID rows the row -> segment map holds
+__host__ __device__ constexpr uint32_t dedup_ld_bytes() { return kLdMaxProbe * 4 + (kLdMaxProbe + 4) * 4 + kLdRowMap * 2; }
+// first ID of grid cell g (g = kGridCells: N)
+__host__ __device__ inline uint32_t grid_start(uint64_t N, uint32_t g) { return (uint32_t)((N * g) / kGridCells); }
 
 // Partition of a query's valid IDs into S classes (both the partition kernel and the dedup kernel's own
 // filter use these, so a class means the same set of IDs wherever it is computed):
@@ -602,7 +624,7 @@ __host__ __device__ constexpr uint32_t dedup_table_off(uint32_t shape) { return 
 // bucket order into the query's distinct list.
 // T threads per CTA: 1024 (one CTA per SM, the whole shared memory as one table) or 512 (two CTAs per SM with half
 // the table each: one computes while the other waits at a barrier).
-template <int T, int R>
+template <int T, int R, bool LD = false>
 __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const DedupParams p)
 {
     constexpr int BS = kDedupBucketSlots, BSH = BS == 1 ? 2 : BS == 2 ? 3 : 4;   // slots per bucket, log2 of its bytes
@@ -616,7 +638,11 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
     uint32_t *misc = reinterpret_cast<uint32_t *>(smem);
     uint32_t *wsum = misc + 32, *qcnt = misc + 2;
     uint2 *queue = reinterpret_cast<uint2 *>(smem + 256);                    // two retry queues of QCAP (id, bucket address)
-    uint32_t *table = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T * R / 8));
+    // lists-direct: segment starts, prefix of segment lengths, row -> segment map, between the queues and the table
+    uint32_t *seg_start = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T * R / 8));
+    uint32_t *seg_prefix = seg_start + kLdMaxProbe;
+    uint16_t *row_map = reinterpret_cast<uint16_t *>(seg_prefix + kLdMaxProbe + 4);
+    uint32_t *table = reinterpret_cast<uint32_t *>(smem + dedup_table_off(T * R / 8) + (LD ? dedup_ld_bytes() : 0u));
     const uint32_t tbl = (uint32_t)__cvta_generic_to_shared(table);
     const uint32_t none_addr = (uint32_t)__cvta_generic_to_shared(misc + 16);   // a bucket that always holds 4 x kEmpty
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -632,7 +658,9 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
         const uint32_t b = it.x, part = it.y, S = p.S[b];
         const long long Cll = p.cand_offsets[b + 1] - p.cand_offsets[b];
         const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;       // plan guarantees C / S <= 0.75 nslots_max
-        const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
+        const bool ordered = p.mode[b] != kModeHashed;
+        // lists-direct, ordered: bucket_cnt holds the class's exact ID count (lists_classes_kernel)
+        const bool pre = LD ? ordered : (p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0);
         // table sized to the partition, never more than the CTA can hold: 2 slots per expected candidate; 1.5
         // where the count is exact (about 0.4 full after dedup)
         uint32_t nslots = p.nslots_max;
@@ -643,10 +671,15 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
         // ordered mode: this partition owns the IDs of class `part`, a range [lo, lo + span);
         // bucket = (id - lo) * nb / span
         uint32_t lo = 0, span = 0, bmul = 0;
-        if (p.mode[b] != kModeHashed) {
-            const uint32_t class_mul = ordered_class_mul(p.N, S);
-            lo = ordered_class_start(class_mul, part, p.N);
-            span = ordered_class_start(class_mul, part + 1, p.N) - lo;
+        if (ordered) {
+            if (LD) {                                          // classes are runs of grid cells (S divides kGridCells)
+                lo = grid_start(p.N, part * (kGridCells / S));
+                span = grid_start(p.N, (part + 1) * (kGridCells / S)) - lo;
+            } else {
+                const uint32_t class_mul = ordered_class_mul(p.N, S);
+                lo = ordered_class_start(class_mul, part, p.N);
+                span = ordered_class_start(class_mul, part + 1, p.N) - lo;
+            }
             // span <= nb (tiny N): bucket = id - lo - 1 or 0, still order-preserving and inside the table
             bmul = span > nb ? (uint32_t)(((unsigned long long)nb << 32) / span) : 0xFFFFFFFFu;
         }
@@ -676,21 +709,92 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
         const long long Cll = p.cand_offsets[b + 1] - off0;
         const uint32_t C = Cll > 0 ? (uint32_t)Cll : 0u;
         // pre-partitioned: this item's IDs were split off by partition_kernel; every ID read is ours
-        const bool pre = p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
+        const bool pre = !LD && p.part_ids != nullptr && S > 1 && p.part_ok[b] != 0;
         const uint32_t Cin = pre ? p.bucket_cnt[item] : C;     // IDs this pass reads
 
         // candidate list as 16-byte vectors; vector 0 may start up to 3 elements before the list.
         // Vectors [v_in0, v_in1) lie wholly inside the list and are read with one 16-byte load.
         const uint32_t *ids = pre ? p.part_ids + 2 * off0 + (size_t)part * (uint32_t)(2ull * C / S) : p.cand_ids + off0;
-        const uint32_t shift = (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
+        const uint32_t shift = LD ? 0u : (uint32_t)((reinterpret_cast<uintptr_t>(ids) >> 2) & 3u);
         const uint4 *ids4 = reinterpret_cast<const uint4 *>(ids - shift);
-        const uint32_t nvec = Cin ? (Cin + shift + 3u) >> 2 : 0u;
+        uint32_t nvec = Cin ? (Cin + shift + 3u) >> 2 : 0u;
         const uint32_t v_in0 = shift ? 1u : 0u, v_in1 = (Cin + shift) >> 2;
         const uint4 none4 = make_uint4(kIdNone, kIdNone, kIdNone, kIdNone);
+        uint32_t ld_total = 0;                                 // lists-direct: IDs of this item's segments
+        if constexpr (LD) {
+            // The item's IDs are one segment of every probed list: the whole list (hashed classes), or its IDs of
+            // this ID-range class, bounded by two entries of the list's grid.  Segment table, prefix of the
+            // lengths, and for every 32 positions of the concatenation the segment its first position is in.
+            const uint32_t w = hashed ? 0u : kGridCells / S;
+            uint32_t len = 0;
+            if (tid < p.nprobe) {
+                const uint32_t l = __ldg(p.probes + (size_t)b * p.nprobe + tid);
+                if ((uint64_t)l < p.n_lists) {
+                    const uint16_t *g = p.list_grid + (size_t)l * (kGridCells + 1);
+                    const uint32_t a = hashed ? 0u : __ldg(g + part * w), e = hashed ? __ldg(g + kGridCells) : __ldg(g + (part + 1) * w);
+                    seg_start[tid] = (uint32_t)(__ldg(p.list_offsets + l) + a);
+                    len = e - a;
+                }
+            }
+            uint32_t incl = len;                               // block exclusive scan of the lengths
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += u;
+            }
+            if (lane == 31) wsum[warp] = incl;
+            __syncthreads();
+            if (warp == 0) {
+                const uint32_t wv = lane < T / 32 ? wsum[lane] : 0u;
+                uint32_t wi = wv;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t u = __shfl_up_sync(0xffffffffu, wi, o);
+                    if (lane >= o) wi += u;
+                }
+                wsum[lane] = wi - wv;
+                if (lane == 31) misc[6] = wi;                  // IDs of the item
+            }
+            __syncthreads();
+            const uint32_t ex = wsum[warp] + incl - len;
+            ld_total = misc[6];
+            if (tid < p.nprobe) seg_prefix[tid] = ex;
+            if (tid == 0) seg_prefix[p.nprobe] = ld_total;
+            if (len) {                                         // rows whose first position lies in this segment
+                for (uint32_t r = (ex + 31u) >> 5; (r << 5) < ex + len; ++r)
+                    if (r < kLdRowMap) row_map[r] = (uint16_t)tid;
+            }
+            nvec = ((ld_total + 127u) >> 7) << 5;              // groups of 32 vectors = 128 positions
+            __syncthreads();
+        }
         auto load_vec = [&](uint32_t v) -> uint4 {
-            if (v >= v_in0 && v < v_in1) return __ldg(ids4 + v);
-            if (v < nvec) return load_ids4(ids, 4ll * v - shift, Cin);
-            return none4;
+            if constexpr (LD) {
+                // vectors 32 g .. 32 g + 31 (one warp) cover positions [128 g, 128 g + 128) of the concatenated
+                // segments; element e of lane l is position 128 g + 32 e + l, so every load of a warp is contiguous
+                uint32_t x[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t q = ((v >> 5) << 7) + 32u * e + (v & 31u);
+                    x[e] = kIdNone;
+                    if (q < ld_total) {
+                        uint32_t sg;
+                        if ((q >> 5) < kLdRowMap) {
+                            sg = row_map[q >> 5];
+                        } else {                               // beyond the row map (hashed classes read whole lists): search
+                            uint32_t lo_s = 0, hi_s = p.nprobe;
+                            while (hi_s - lo_s > 1) { const uint32_t mid = (lo_s + hi_s) >> 1; if (seg_prefix[mid] <= q) lo_s = mid; else hi_s = mid; }
+                            sg = lo_s;
+                        }
+                        while (q >= seg_prefix[sg + 1]) ++sg;  // also skips empty segments
+                        x[e] = __ldg(p.list_ids + seg_start[sg] + (q - seg_prefix[sg]));
+                    }
+                }
+                return make_uint4(x[0], x[1], x[2], x[3]);
+            } else {
+                if (v >= v_in0 && v < v_in1) return __ldg(ids4 + v);
+                if (v < nvec) return load_ids4(ids, 4ll * v - shift, Cin);
+                return none4;
+            }
         };
         // hashed mode: bucket and home slot of a valid ID
         auto hash_of = [&](uint32_t x) -> uint32_t {

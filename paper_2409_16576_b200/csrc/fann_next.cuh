@@ -144,6 +144,89 @@ __global__ void __launch_bounds__(kExpandThreads) lists_expand_kernel(const long
     }
 }
 
+// ---------------------------------------------------------------- lists-direct: sorted lists + grid
+
+constexpr uint32_t kSortMaxList = 8192;               // longest list lists_sort_grid_kernel sorts (in shared memory)
+
+// fann_load_lists: one CTA per posting list.  Sorts the list's IDs ascending in place (set semantics: the order of a
+// list's IDs carries no meaning) and writes its grid: grid[l][g] = position of the first ID >=
+// grid_start(N, g), g = 0 .. kGridCells (the last entry = number of valid IDs; IDs >= N and padding sort behind it).
+// A list longer than kSortMaxList is left as it is and *unsorted is raised (the direct path is then not used).
+__global__ void __launch_bounds__(256) lists_sort_grid_kernel(const long long *__restrict__ list_offsets, uint32_t *list_ids,
+                                                              uint64_t N, uint16_t *__restrict__ grid, uint32_t *unsorted)
+{
+    extern __shared__ uint32_t sm_ids[];
+    const uint32_t l = blockIdx.x, tid = threadIdx.x;
+    const long long o0 = list_offsets[l];
+    const long long Lll = list_offsets[l + 1] - o0;
+    uint16_t *g = grid + (size_t)l * (kGridCells + 1);
+    if (Lll < 0 || Lll > (long long)kSortMaxList) {
+        if (tid == 0) atomicExch(unsorted, 1u);
+        if (tid <= kGridCells) g[tid] = 0;
+        return;
+    }
+    const uint32_t L = (uint32_t)Lll;
+    uint32_t P = 32;
+    while (P < L) P <<= 1;
+    for (uint32_t i = tid; i < P; i += 256) sm_ids[i] = i < L ? list_ids[o0 + i] : 0xFFFFFFFFu;
+    __syncthreads();
+    for (uint32_t size = 2; size <= P; size <<= 1)
+        for (uint32_t stride = size >> 1; stride > 0; stride >>= 1) {
+            for (uint32_t i = tid; i < (P >> 1); i += 256) {
+                const uint32_t lo = 2 * i - (i & (stride - 1)), hi = lo + stride;
+                const bool asc = (lo & size) == 0;
+                const uint32_t x = sm_ids[lo], y = sm_ids[hi];
+                if ((x > y) == asc) { sm_ids[lo] = y; sm_ids[hi] = x; }
+            }
+            __syncthreads();
+        }
+    for (uint32_t i = tid; i < L; i += 256) list_ids[o0 + i] = sm_ids[i];
+    if (tid <= kGridCells) {
+        const uint64_t bound = tid == kGridCells ? N : (uint64_t)grid_start(N, tid);
+        uint32_t lo = 0, hi = L;                              // first position with id >= bound
+        while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if ((uint64_t)sm_ids[mid] < bound) lo = mid + 1; else hi = mid; }
+        g[tid] = (uint16_t)lo;
+    }
+}
+
+// Lists-direct, one CTA per query, after plan_kernel fixed S_b (a power of two): the exact number of IDs of every
+// ID-range class, from the grids of the probed lists.  Ordered placement if every class fits a dedup table even if
+// none of its IDs repeats, else hash classes (which read whole lists).  bucket_cnt[item] = the class's ID count.
+__global__ void __launch_bounds__(256) lists_classes_kernel(const uint16_t *__restrict__ grid, uint64_t n_lists, uint64_t N,
+                                                            const uint32_t *__restrict__ probes, uint32_t nprobe,
+                                                            const uint32_t *__restrict__ S, const uint32_t *__restrict__ item_start,
+                                                            uint32_t class_max, uint32_t force, uint32_t *__restrict__ mode,
+                                                            uint32_t *__restrict__ bucket_cnt)
+{
+    __shared__ uint32_t tot[kGridCells];
+    const uint32_t b = blockIdx.x, tid = threadIdx.x, Sb = S[b];
+    if (tid < kGridCells) tot[tid] = 0;
+    __syncthreads();
+    const bool can_order = Sb >= 1 && Sb <= kGridCells && (Sb & (Sb - 1)) == 0 && N >= 4096 && force != kModeHashed;
+    if (can_order) {
+        const uint32_t w = kGridCells / Sb;
+        for (uint32_t j = tid; j < nprobe; j += 256) {
+            const uint32_t l = __ldg(probes + (size_t)b * nprobe + j);
+            if ((uint64_t)l >= n_lists) continue;
+            const uint16_t *g = grid + (size_t)l * (kGridCells + 1);
+            uint32_t prev = __ldg(g);
+            for (uint32_t c = 0; c < Sb; ++c) {
+                const uint32_t nxt = __ldg(g + (c + 1) * w);
+                if (nxt > prev) atomicAdd(&tot[c], nxt - prev);
+                prev = nxt;
+            }
+        }
+    }
+    __syncthreads();
+    bool big = false;
+    if (can_order && tid < Sb) {
+        big = tot[tid] > class_max;
+        bucket_cnt[item_start[b] + tid] = tot[tid];
+    }
+    big = __syncthreads_or(big);
+    if (tid == 0) mode[b] = (can_order && (!big || force == kModeOrdered)) ? kModeOrdered : kModeHashed;
+}
+
 // List-major experiment: row e of the copy = the code row of the vector list entry e names (zero if it names none).
 __global__ void list_codes_kernel(const uint8_t *__restrict__ codes, uint64_t N, uint32_t row_bytes,
                                   const uint32_t *__restrict__ list_ids, uint64_t e0, uint64_t n, uint8_t *__restrict__ dst)

@@ -65,7 +65,12 @@ def _search_lists(fann, w, probes_np, k=None, cap=None):
     return ix, (np_u32(o[0]), o[1].cpu().numpy(), np_u32(o[2]), np_u32(o[3]))
 
 
-def test_search_lists_equals_oracle_and_the_id_path(fann, wl_int, wl_tiny):
+@pytest.mark.parametrize("direct", ["1", "0"])
+def test_search_lists_equals_oracle_and_the_id_path(fann, wl_int, wl_tiny, monkeypatch, direct):
+    """direct = 1: the lists are sorted and indexed at load and the dedup kernel reads every ID-range class straight
+    from the probed lists; 0 (FANN_LISTS_DIRECT=0, also the path of lists too long to sort): the candidate array is
+    written out and split first.  Same bytes either way."""
+    monkeypatch.setenv("FANN_LISTS_DIRECT", direct)
     for w in (wl_int, wl_tiny):
         P = w.probes.numpy().view(np.uint32)
         ix, res = _search_lists(fann, w, P)
@@ -94,7 +99,11 @@ def test_search_lists_equals_oracle_and_the_id_path(fann, wl_int, wl_tiny):
         ix.close()
 
 
-def test_search_lists_padding_unknown_lists_and_capacity(fann, wl_int):
+@pytest.mark.parametrize("env", [{}, {"FANN_DEDUP_MODE": "1"}, {"FANN_DEDUP_THREADS": "1024"}, {"FANN_LISTS_DIRECT": "0"}])
+def test_search_lists_padding_unknown_lists_and_capacity(fann, wl_int, monkeypatch, env):
+    """Also with hash classes forced (the direct path then reads whole lists and filters) and with the one-CTA shape."""
+    for key, val in env.items():
+        monkeypatch.setenv(key, val)
     w = wl_int
     P = w.probes.numpy().view(np.uint32).copy()
     P[0, ::2] = NONE                                             # padding probes
