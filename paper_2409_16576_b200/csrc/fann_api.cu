@@ -56,6 +56,7 @@ struct fann_index {
     uint32_t dedup_smem_half = 0;          // same for two CTAs per SM
     uint32_t dedup_threads = 0;            // 0: chosen per call (geometry()); 1024 or 512: forced (FANN_DEDUP_THREADS)
     std::atomic<uint64_t> launches{0};
+    std::atomic<uint32_t> generation{0};   // bumped by the loaders: captured graphs (fann_pool) hold the arrays' addresses
     // everything below is shared by concurrent callers and guarded by `mu`
     std::mutex mu;
     std::vector<CallCtx *> ctx_pool;       // idle call contexts
@@ -320,6 +321,7 @@ extern "C" int fann_load_codes(fann_index *ix, const uint8_t *codes, uint64_t fi
                                                             (unsigned long long)first, (unsigned long long)n, (unsigned long long)N_total);
     DeviceGuard guard(ix->device);
     cudaStream_t stream = (cudaStream_t)stream_;
+    ix->generation++;
     if (!ix->codes) {
         ix->N = N_total; ix->M = M; ix->row_bytes = stored_row_bytes(M);
         cudaError_t e = cudaMalloc(&ix->codes, (size_t)N_total * ix->row_bytes);
@@ -789,6 +791,7 @@ extern "C" int fann_load_lists(fann_index *ix, const int64_t *list_offsets, cons
         return fail(FANN_EINVAL, "fann_load_lists: list_offsets must be 8-byte and list_ids 4-byte aligned");
     DeviceGuard guard(ix->device);
     cudaStream_t stream = (cudaStream_t)stream_;
+    ix->generation++;
     if (ix->list_offsets) { cudaFree(ix->list_offsets); ix->list_offsets = nullptr; }
     if (ix->list_ids) { cudaFree(ix->list_ids); ix->list_ids = nullptr; }
     if (ix->lm_codes) { cudaFree(ix->lm_codes); ix->lm_codes = nullptr; }      // built from the old lists
@@ -1143,7 +1146,7 @@ struct fann_pool {
     std::vector<cudaStream_t> streams;
     // CUDA graphs of the posting-list form (one per block and call shape): the ten kernel launches and five copies of
     // a call replayed by one cudaGraphLaunch from the block's pinned staging buffer
-    struct Graph { uint32_t B, nprobe, k; const float *codebooks; cudaGraphExec_t exec; };
+    struct Graph { uint32_t B, nprobe, k, generation; const float *codebooks; cudaGraphExec_t exec; };
     std::vector<std::vector<Graph>> graphs;        // per block; a block is used by one call at a time
     char *staging = nullptr;                       // pinned host memory, staging_bytes per block
     size_t staging_bytes = 0, st_queries = 0, st_probes = 0, st_ids = 0, st_dists = 0, st_counts = 0, st_hdr = 0;
@@ -1303,7 +1306,13 @@ extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const fl
     ListsLayout l;
     lists_layout(ix, B, pool->max_cands, k, &l);
     cudaGraphExec_t exec = nullptr;
-    for (auto &g : pool->graphs[lease.id])
+    const uint32_t gen = ix->generation.load();
+    auto &cache = pool->graphs[lease.id];
+    for (size_t i = 0; i < cache.size();) {                    // graphs captured before codes or lists were reloaded are stale
+        if (cache[i].generation != gen) { cudaGraphExecDestroy(cache[i].exec); cache.erase(cache.begin() + i); }
+        else ++i;
+    }
+    for (auto &g : cache)
         if (g.B == B && g.nprobe == nprobe && g.k == k && g.codebooks == codebooks_d) exec = g.exec;
     if (!exec) {
         CUDA_TRY(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
@@ -1330,7 +1339,7 @@ extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const fl
         ce = cudaGraphInstantiate(&exec, graph, 0);
         cudaGraphDestroy(graph);
         if (ce != cudaSuccess) return fail(FANN_ECUDA, "fann_search_small_lists: cudaGraphInstantiate: %s", cudaGetErrorString(ce));
-        pool->graphs[lease.id].push_back({B, nprobe, k, codebooks_d, exec});
+        cache.push_back({B, nprobe, k, gen, codebooks_d, exec});
     }
     CUDA_TRY(cudaGraphLaunch(exec, stream));
     CUDA_TRY(cudaStreamSynchronize(stream));

@@ -774,19 +774,25 @@ __global__ void __launch_bounds__(T, 1024 / (T * R / 8)) dedup_kernel(const Dedu
                 uint32_t x[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const uint32_t q = ((v >> 5) << 7) + 32u * e + (v & 31u);
+                    const uint32_t q0 = ((v >> 5) << 7) + 32u * e, q = q0 + (v & 31u);   // the row's first position: warp-uniform
                     x[e] = kIdNone;
-                    if (q < ld_total) {
+                    if (q0 < ld_total) {
                         uint32_t sg;
-                        if ((q >> 5) < kLdRowMap) {
-                            sg = row_map[q >> 5];
+                        if ((q0 >> 5) < kLdRowMap) {
+                            sg = row_map[q0 >> 5];
                         } else {                               // beyond the row map (hashed classes read whole lists): search
                             uint32_t lo_s = 0, hi_s = p.nprobe;
-                            while (hi_s - lo_s > 1) { const uint32_t mid = (lo_s + hi_s) >> 1; if (seg_prefix[mid] <= q) lo_s = mid; else hi_s = mid; }
+                            while (hi_s - lo_s > 1) { const uint32_t mid = (lo_s + hi_s) >> 1; if (seg_prefix[mid] <= q0) lo_s = mid; else hi_s = mid; }
                             sg = lo_s;
                         }
-                        while (q >= seg_prefix[sg + 1]) ++sg;  // also skips empty segments
-                        x[e] = __ldg(p.list_ids + seg_start[sg] + (q - seg_prefix[sg]));
+                        if (q0 + 31u >= seg_prefix[sg + 1]) {  // the row runs into later segments: every lane finds its own
+                            if (q < ld_total) {
+                                while (q >= seg_prefix[sg + 1]) ++sg;   // also skips empty segments
+                                x[e] = __ldg(p.list_ids + seg_start[sg] + (q - seg_prefix[sg]));
+                            }
+                        } else {
+                            x[e] = __ldg(p.list_ids + (seg_start[sg] + (q - seg_prefix[sg])));
+                        }
                     }
                 }
                 return make_uint4(x[0], x[1], x[2], x[3]);

@@ -138,6 +138,16 @@ def test_pool_entries_match_the_oracle(fann, wl, ref, monkeypatch, graphs):
             assert np.array_equal(oc, r["counts"])
     st = fann.fann_pool_stats(pool)
     assert st["calls"] == 12 and st["in_use"] == 0 and st["n_blocks"] == 2 and st["high_water"] == 1
+    # other posting lists loaded under a live pool: graphs captured for the old arrays must not be replayed
+    ids2 = torch.flip(w.list_ids, dims=[0]).contiguous()
+    ix.load_lists(w.list_offsets.to(DEV), ids2.to(DEV))
+    P = np.ascontiguousarray(w.probes[:3].numpy())
+    oi, od, oc = np.zeros((3, k), np.uint32), np.zeros((3, k), np.float32), np.zeros(3, np.uint32)
+    fann.fann_search_small_lists(ix.handle, pool, w.queries[:3].contiguous().numpy(), 3, cb, w.cfg.dsub, P, w.cfg.nprobe, k, oi, od, oc)
+    r2 = oracle.search_lists(w.queries[:3].numpy(), w.codebooks.numpy(), w.codes.numpy(), w.list_offsets.numpy(),
+                             ids2.numpy(), P.view(np.uint32), k)
+    assert np.array_equal(oi, r2["ids"]) and np.array_equal(oc, r2["counts"])
+    ix.load_lists(w.list_offsets.to(DEV), w.list_ids.to(DEV))
     # what the pool was not created for
     q, off, ids = _sub(w, 0, 5)
     oi, od, oc = np.zeros((5, k), np.uint32), np.zeros((5, k), np.float32), np.zeros(5, np.uint32)
