@@ -311,9 +311,56 @@ def probe_sweep(args, cfg):
                torch.randint(0, page_rows, (n,), device=dev, generator=gen)).to(torch.int32)
         pages_test.append({"pages_2MB": int(K), "footprint_GB": round(K * (2 << 20) / 1e9, 2),
                            "G_rows_per_s": rate(ids, 3, 1)})
+    # what about the order matters: the same kind of lists (one per CTA, U random rows), cp.async ring, 1 CTA per SM
+    n_st = U // unit
+
+    def rnd_perm(*shape):
+        return torch.argsort(torch.rand(shape, device=dev, generator=gen), dim=-1)
+
+    def ordered(variant):
+        out = []
+        for _ in range(groups):
+            ids = torch.randint(0, N, (sms, U), device=dev, generator=gen, dtype=torch.int64).sort(dim=1).values
+            if variant == "ascending_each_cta_at_another_phase":
+                sh = (torch.arange(sms, device=dev) * n_st // sms) * unit
+                ids = torch.gather(ids, 1, (torch.arange(U, device=dev)[None, :] + sh[:, None]) % U)
+            elif variant == "cta_steps_shuffled_ascending_inside":          # a step = the 16 warps' stages: `unit` rows
+                p = rnd_perm(sms, n_st)
+                ids = torch.gather(ids.view(sms, n_st, unit), 1, p[:, :, None].expand(-1, -1, unit)).reshape(sms, U)
+            elif variant == "cta_steps_ascending_shuffled_inside":
+                ids = torch.gather(ids.view(sms, n_st, unit), 2, rnd_perm(sms, n_st, unit)).reshape(sms, U)
+            elif variant == "warp_stage_rows_in_random_lane_order":
+                ids = torch.gather(ids.view(sms, U // rps, rps), 2, rnd_perm(sms, U // rps, rps)).reshape(sms, U)
+            elif variant == "rows_of_a_step_dealt_round_robin_to_warps":
+                ids = ids.view(sms, n_st, rps, 16).permute(0, 1, 3, 2).reshape(sms, U)
+            elif variant.startswith("warp_stage_random_in_window_MB_"):     # a stage's rows random inside a window at a random place
+                X = int(variant.rsplit("_", 1)[1]) << 20
+                base = torch.randint(0, (N * row_bytes - X) // row_bytes, (sms, U // rps), device=dev, generator=gen)
+                ids = base.repeat_interleave(rps, dim=1) + torch.randint(0, X // row_bytes, (sms, U), device=dev, generator=gen)
+            elif variant == "each_warp_instruction_in_its_own_random_2MB_page":
+                per = 512 // row_bytes                                      # rows one 32-lane 16-byte instruction covers
+                pg = torch.randint(0, npages, (sms, U // per), device=dev, generator=gen)
+                ids = pg.repeat_interleave(per, dim=1) * page_rows + torch.randint(0, page_rows, (sms, U), device=dev, generator=gen)
+            elif variant.startswith("share_with_neighbour_cta_pct_"):       # L2: a part of every list is the next CTA's rows too
+                kk = U * int(variant.rsplit("_", 1)[1]) // 100
+                nb = torch.gather(torch.roll(ids, 1, 0), 1, rnd_perm(sms, U)[:, :kk])
+                ids = torch.cat([torch.gather(ids, 1, rnd_perm(sms, U)[:, : U - kk]), nb], 1).sort(dim=1).values
+            elif variant == "random":
+                ids = torch.gather(ids, 1, rnd_perm(sms, U))
+            out.append(ids.view(sms, n_st, 16, rps).permute(1, 0, 2, 3).reshape(-1))
+        return torch.cat(out).to(torch.int32).contiguous()
+
+    order_study = []
+    for variant in ("ascending", "ascending_each_cta_at_another_phase", "cta_steps_shuffled_ascending_inside",
+                    "cta_steps_ascending_shuffled_inside", "warp_stage_rows_in_random_lane_order",
+                    "rows_of_a_step_dealt_round_robin_to_warps", "each_warp_instruction_in_its_own_random_2MB_page",
+                    "warp_stage_random_in_window_MB_8", "warp_stage_random_in_window_MB_128",
+                    "warp_stage_random_in_window_MB_512", "warp_stage_random_in_window_MB_2048",
+                    "share_with_neighbour_cta_pct_30", "share_with_neighbour_cta_pct_60", "random"):
+        order_study.append({"order": variant, "G_rows_per_s": rate(ordered(variant), 3, 1)})
     print(json.dumps({"probe_sweep": {"workload": cfg.name, "N": N, "row_bytes": row_bytes, "array_GB": round(N * row_bytes / 1e9, 1),
                                       "rows_per_cta_list": U, "sms": sms, "order_x_flavor": sweep,
-                                      "random_rows_in_K_pages": pages_test}}))
+                                      "random_rows_in_K_pages": pages_test, "order_study": order_study}}))
 
 
 def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=False, sample_clocks=False):
@@ -323,7 +370,15 @@ def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=F
     import torch
     from workloads import DEFAULT_SEED, make_workload
     t_gen = time.time()
-    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev, keep_lists=keep_lists)   # each replica: its own batch
+    by_window = getattr(args, "query_order", "generated") == "window"
+    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev, keep_lists=keep_lists or by_window)   # each replica: its own batch
+    if by_window:
+        # measurement variant: the same queries, ordered by the position of their probed window, so that queries
+        # which share posting lists -- and code rows -- are scanned at about the same time (L2 reuse)
+        from workloads.generate import PostingLists, make_candidates
+        perm = torch.argsort(w.probes.long().median(dim=1).values)
+        w.probes, w.queries = w.probes[perm].contiguous(), w.queries[perm].contiguous()
+        w.cand_offsets, w.cand_ids = make_candidates(cfg, PostingLists(w.list_offsets, w.list_ids, 0), w.probes.long())
     torch.cuda.synchronize()
     t_gen = time.time() - t_gen
     B, k, M, dsub = cfg.B, cfg.k, cfg.M, cfg.dsub
@@ -515,6 +570,76 @@ def list_major_leg(fann, ix, w, cfg, args, dev, ref_ids, U_total, C_total):
             "matches_device_path": same_ids(cfg, oi.cpu().numpy(), ref_ids)}
 
 
+def next_rows_leg(fann, cfg, live, dev, args, with_oracle: bool):
+    """SURVEY.md 8(f) NEXT-1 and NEXT-4 measured where the raw vectors fit beside the codes (configs[1], the
+    paper's SIFT-shaped case): Algorithm 1 re-ranks the GPU stage's top-n of every query of
+    the batch just timed, then Fig. 8's page plan (L198) for the mini-batches Algorithm 1 executed.  CUDA events
+    around fann_rerank / fann_page_reads; algorithmic bytes of the re-ranking = raw vectors read + tasks +
+    queries + outputs.  The kernels wait on one dependent row gather per mini-batch (the stop rule decides
+    whether the next mini-batch is read at all), so this is a latency-bound step: the HBM fraction says so."""
+    import numpy as np
+    import torch
+    from workloads import DEFAULT_SEED, make_page_table, make_raw_vectors
+    w, ix, out = live["w"], live["ix"], live["out"]
+    B, n = out[0].shape
+    vec = make_raw_vectors(cfg, DEFAULT_SEED, device=dev)
+    page_of, n_pages = make_page_table(cfg, DEFAULT_SEED, device=dev, elem_bytes=vec.element_size())
+    ix.load_vectors(vec)
+    ix.load_page_table(page_of, n_pages)
+    tasks = out[0]
+    peak, _ = measured_peak_gbs()
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+
+    def timed(fn):
+        for _ in range(max(3, args.warmup)):
+            r = fn()
+        ms = 0.0
+        for i in range(args.steps):
+            flush.fill_(i & 0xFF)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            r = fn()
+            b.record()
+            b.synchronize()
+            ms += a.elapsed_time(b)
+        return ms / args.steps, r
+
+    legs = []
+    for bs, k, eps, beta in ((10, 10, 0.15, 2), (10, 10, 0.0, 1)):
+        ms, got = timed(lambda: ix.rerank(w.queries, tasks, bs, k, eps, beta))
+        reads = int(got[4].sum().item())
+        byts = reads * cfg.d * vec.element_size() + tasks.numel() * 4 + B * cfg.d * 4 + B * k * 8
+        leg = {"n": n, "batch_size": bs, "k": k, "eps": eps, "beta": beta, "ms": round(ms, 4),
+               "queries_per_s": B / (ms * 1e-3), "raw_vectors_read_per_query": reads / B,
+               "mini_batches_per_query": float(got[3].float().mean().item()),
+               "algorithmic_bytes": byts, "GB_per_s": round(byts / ms / 1e6, 1), "hbm_frac": round(byts / ms / 1e6 / peak, 4)}
+        if with_oracle:
+            import oracle
+            nq = min(B, 32)
+            used, rel = torch.unique(tasks[:nq].reshape(-1), return_inverse=True)
+            rows = vec[used.long()].cpu().numpy().astype(np.float32)
+            ref = oracle.rerank(w.queries[:nq].cpu().numpy(), rows, rel.view(nq, n).cpu().numpy().astype(np.uint32), bs, k, eps, beta)
+            ids = used.cpu().numpy().view(np.uint32)[ref["ids"]]
+            leg["matches_oracle_on_sample"] = bool(
+                np.array_equal(got[0][:nq].cpu().numpy().view(np.uint32), ids) and
+                np.array_equal(got[3][:nq].cpu().numpy().view(np.uint32), ref["batches"]) and
+                np.allclose(got[1][:nq].cpu().numpy(), ref["dists"], rtol=1e-5, atol=0))
+        pms, pr = timed(lambda: ix.page_reads(tasks, bs, batches_run=got[3]))
+        leg["page_reads"] = {"ms": round(pms, 4), "queries_per_s": B / (pms * 1e-3),
+                             "pages_per_query": float(pr[2].float().mean().item()),
+                             "tasks_per_s": reads / (pms * 1e-3)}
+        if with_oracle:
+            pg, br, tot = oracle.page_reads(page_of.cpu().numpy().view(np.uint32), tasks[:nq].cpu().numpy().view(np.uint32),
+                                            bs, max_batches=ref["batches"])
+            leg["page_reads"]["matches_oracle_on_sample"] = bool(
+                np.array_equal(pr[2][:nq].cpu().numpy().view(np.uint32), tot) and
+                np.array_equal(pr[1][:nq].cpu().numpy().view(np.uint32), br))
+        legs.append(leg)
+    del vec, page_of, flush
+    return {"workload": cfg.name, "raw_vectors": f"[{cfg.N}][{cfg.d}] {cfg.values} in HBM", "l2": "flushed between timed calls",
+            "entries": "fann_rerank (Algorithm 1), fann_page_reads (Fig. 8)", "runs": legs}
+
+
 def sample_parity(w, cfg, out, nq):
     """GPU output of the first nq queries against the CPU oracle (bytes for integer data, the 1e-5 band else).
     Returns (parity flag, seconds the oracle took, oracle result, distinct candidates scored)."""
@@ -549,6 +674,8 @@ def main():
     ap.add_argument("--no-experiment", action="store_true", help="skip the list-major streaming experiment")
     ap.add_argument("--probe-sweep", action="store_true",
                     help="measurement only: the row-gather ceiling sweep on a synthetic array of the workload's size")
+    ap.add_argument("--query-order", default="generated", choices=["generated", "window"],
+                    help="measurement variant: 'window' orders the batch's queries by the position of their probed lists")
     ap.add_argument("--id-map", default=None, choices=["feistel", "lattice"],
                     help="vector -> ID map of the generator (default: the config's, 'feistel')")
     args = ap.parse_args()
@@ -686,7 +813,7 @@ def main():
     stats = res["stats"]
 
     # ---- the other large workloads ("report both" 1B configs), same process, one after another
-    others = None
+    others, next_rows = None, None
     if world == 1 and not args.no_configs and args.workload == DEFAULT_WORKLOAD:
         live.clear()
         ix.close()
@@ -706,6 +833,11 @@ def main():
                 par, dt, _, units = sample_parity(l2["w"], c2, l2["out"], min(c2.B, 48))
                 entry["gpu_matches_oracle_on_sample"] = par
                 entry["oracle_sample"] = f"first {min(c2.B, 48)} queries, {units} distinct candidates, {dt:.2f} s"
+            if name == "u8_10m_m32":
+                try:
+                    next_rows = next_rows_leg(fann, c2, l2, dev, args, with_oracle=not args.no_cpu)
+                except Exception as e:                              # never take the bench line down
+                    next_rows = {"error": str(e)[:200]}
             others.append(entry)
             l2["ix"].close()
             l2.clear()
@@ -718,7 +850,7 @@ def main():
         "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "N": cfg.N, "d": cfg.d, "M": M, "B": B, "nprobe": cfg.nprobe, "k": k,
-                   "id_map": cfg.id_map, "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
+                   "id_map": cfg.id_map, "query_order": args.query_order, "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                    "l2": res["l2"], "C_total": total, "U_total": U_total,
                    "distinct_fraction": round(U_total / max(total, 1), 4),
                    "C_mean": stats["C_mean"], "C_max": stats["C_max"], "gen_seconds": res["gen_seconds"]},
@@ -726,7 +858,7 @@ def main():
         "input_ids_per_s": res["C_all"] / (ms_per_step * 1e-3),
         "hbm_frac_nominal_8TBs": round(roofline["achieved"] / 8000.0, 4),
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_candidate_ids": e2e_ids, "small_batch": small,
-        "experiment_list_major": experiment,
+        "experiment_list_major": experiment, "next_rows": next_rows,
         "gpu_launches": res["launches"], "clocks": res["clocks"], "geometry": geometry, "configs": others,
     }
     print(json.dumps(line))

@@ -96,10 +96,83 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
-// Block-wide bitonic sort (ascending) of n = 2^p keys in shared memory,
-// starting from sorted runs of length first_size / 2.
+// Compare-exchange of the keys at a lower (a) and a higher (b) index of a bitonic network.
+__device__ __forceinline__ void cmpex(unsigned long long &a, unsigned long long &b, bool asc)
+{
+    const bool sw = (a > b) == asc;
+    const unsigned long long t = a;
+    a = sw ? b : a;
+    b = sw ? t : b;
+}
+
+// The steps of merge size `size` with strides s_hi, s_hi / 2, ..., 1 (s_hi <= 64) on the 128 keys a warp holds, four
+// consecutive keys per lane (key r of the lane = element e0 + r): strides 64 ... 4 by shuffles, 2 and 1 in registers.
+__device__ __forceinline__ void bitonic_warp_steps(unsigned long long (&k)[4], uint32_t e0, uint32_t size, uint32_t s_hi)
+{
+    const uint32_t lane = threadIdx.x & 31;
+    const bool asc = (e0 & size) == 0;                         // the same for the lane's four keys when size >= 4
+    for (uint32_t stride = s_hi; stride >= 4; stride >>= 1) {
+        const uint32_t L = stride >> 2;
+        const bool take_min = ((lane & L) == 0) == asc;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const unsigned long long o = __shfl_xor_sync(0xffffffffu, k[r], L);
+            k[r] = ((o < k[r]) == take_min) ? o : k[r];
+        }
+    }
+    if (s_hi >= 2 && size >= 4) { cmpex(k[0], k[2], asc); cmpex(k[1], k[3], asc); }
+    if (size >= 4) { cmpex(k[0], k[1], asc); cmpex(k[2], k[3], asc); }
+    else { cmpex(k[0], k[1], true); cmpex(k[2], k[3], false); }   // size 2: direction = bit 1 of the element index
+}
+
+// Block-wide bitonic sort (ascending) of n = 2^p keys in shared memory, starting from sorted runs of length
+// first_size / 2.  From single keys and n >= 128: every thread keeps four consecutive keys in registers for all
+// steps with stride <= 64 (a warp sorts its 128 keys without touching shared memory or a barrier), and the steps
+// with larger strides go through shared memory two at a time -- 11 barriers instead of 66 for 2048 keys.
 __device__ __forceinline__ void bitonic_sort_smem(unsigned long long *a, uint32_t n, uint32_t first_size)
 {
+    if (first_size == 2 && n >= 128 && (blockDim.x & 31) == 0) {
+        const uint32_t nvt = n >> 2;                           // four keys per (virtual) thread; whole warps
+        for (uint32_t vt = threadIdx.x; vt < nvt; vt += blockDim.x) {
+            unsigned long long k[4] = {a[4 * vt], a[4 * vt + 1], a[4 * vt + 2], a[4 * vt + 3]};
+            for (uint32_t size = 2; size <= 128; size <<= 1) bitonic_warp_steps(k, 4 * vt, size, size >> 1);
+            a[4 * vt] = k[0]; a[4 * vt + 1] = k[1]; a[4 * vt + 2] = k[2]; a[4 * vt + 3] = k[3];
+        }
+        __syncthreads();
+        for (uint32_t size = 256; size <= n; size <<= 1) {
+            uint32_t stride = size >> 1;
+            while (stride >= 128) {
+                if (stride >= 256) {                           // strides `stride` and `stride / 2` in one pass
+                    const uint32_t h = stride >> 1;
+                    for (uint32_t vt = threadIdx.x; vt < nvt; vt += blockDim.x) {
+                        const uint32_t base = ((vt & ~(h - 1)) << 2) | (vt & (h - 1));
+                        const bool asc = (base & size) == 0;
+                        unsigned long long x0 = a[base], x1 = a[base + h], x2 = a[base + stride], x3 = a[base + stride + h];
+                        cmpex(x0, x2, asc); cmpex(x1, x3, asc);
+                        cmpex(x0, x1, asc); cmpex(x2, x3, asc);
+                        a[base] = x0; a[base + h] = x1; a[base + stride] = x2; a[base + stride + h] = x3;
+                    }
+                    stride >>= 2;
+                } else {
+                    for (uint32_t i = threadIdx.x; i < (n >> 1); i += blockDim.x) {
+                        const uint32_t lo = 2 * i - (i & (stride - 1)), hi = lo + stride;
+                        unsigned long long x = a[lo], y = a[hi];
+                        cmpex(x, y, (lo & size) == 0);
+                        a[lo] = x; a[hi] = y;
+                    }
+                    stride >>= 1;
+                }
+                __syncthreads();
+            }
+            for (uint32_t vt = threadIdx.x; vt < nvt; vt += blockDim.x) {
+                unsigned long long k[4] = {a[4 * vt], a[4 * vt + 1], a[4 * vt + 2], a[4 * vt + 3]};
+                bitonic_warp_steps(k, 4 * vt, size, 64);
+                a[4 * vt] = k[0]; a[4 * vt + 1] = k[1]; a[4 * vt + 2] = k[2]; a[4 * vt + 3] = k[3];
+            }
+            __syncthreads();
+        }
+        return;
+    }
     for (uint32_t size = first_size; size <= n; size <<= 1) {
         for (uint32_t stride = size >> 1; stride > 0; stride >>= 1) {
             for (uint32_t i = threadIdx.x; i < (n >> 1); i += blockDim.x) {
@@ -1537,10 +1610,15 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
 
 // Small batches: scan_kernel ran `parts` CTAs per query (a power of two), each on a slice
 // of the query's distinct list; the slices are disjoint, so the query's top-k is the k smallest of the parts' keys.
-// Every part's keys arrive sorted.  One CTA per query merges them pairwise in shared memory: of two ascending
-// lists a, b of K2 keys, min(a[i], b[K2-1-i]) are the K2 smallest of both as a bitonic sequence, which log2(K2)
-// compare-exchange steps sort; log2(parts) such rounds, all pairs of a round side by side.  K2 = power of two >= k.
+// Every part's keys arrive sorted.  One CTA per query, K2 = power of two >= k, all keys in shared memory.
+//   Selection first (parts >= 4): with m = ceil(k / parts), T = the largest of the parts' m-th keys bounds the
+//   k-th smallest key of all from above (every part has m keys <= T, parts * m >= k), so only each part's prefix
+//   of keys <= T can be in the result -- about 1.3 k keys instead of parts * k; they are gathered and sorted.
+//   Otherwise (2 parts, a part with fewer than m keys, or prefixes longer than kMergeSelect keys): pairwise merge --
+//   of two ascending lists a, b of K2 keys, min(a[i], b[K2-1-i]) are the K2 smallest of both as a bitonic
+//   sequence, which log2(K2) compare-exchange steps sort; log2(parts) such rounds, all pairs of a round side by side.
 constexpr int kMergeThreads = 512;
+constexpr uint32_t kMergeSelect = 4096;              // most keys the selection path sorts (8 per thread)
 __global__ void __launch_bounds__(kMergeThreads) merge_parts_kernel(const unsigned long long *__restrict__ part_keys,
                                                                     const uint32_t *__restrict__ uniq_counts, uint32_t q_begin,
                                                                     uint32_t parts, uint32_t k, uint32_t K2, uint32_t *out_ids,
@@ -1548,31 +1626,90 @@ __global__ void __launch_bounds__(kMergeThreads) merge_parts_kernel(const unsign
 {
     extern __shared__ __align__(16) unsigned char smem[];
     unsigned long long *buf = reinterpret_cast<unsigned long long *>(smem);   // [parts][K2]
+    __shared__ unsigned long long s_bound;
+    __shared__ uint32_t s_off[17];
     const uint32_t b = q_begin + blockIdx.x, tid = threadIdx.x;
+    const uint32_t lg = 31u - (uint32_t)__clz(K2);
     const unsigned long long *src = part_keys + (size_t)b * parts * k;
-    for (uint32_t i = tid; i < parts * K2; i += kMergeThreads) {
-        const uint32_t pt = i / K2, j = i - pt * K2;
-        buf[i] = j < k ? src[(size_t)pt * k + j] : kKeyMax;
+    if (tid == 0) s_bound = 0ull;
+    for (uint32_t i0 = tid; i0 < parts * K2; i0 += 8 * kMergeThreads) {     // eight independent loads in flight per thread
+        unsigned long long r[8];
+#pragma unroll
+        for (uint32_t e = 0; e < 8; ++e) {
+            const uint32_t i = i0 + e * kMergeThreads, pt = i >> lg, j = i & (K2 - 1);
+            r[e] = (i < parts * K2 && j < k) ? __ldg(src + (size_t)pt * k + j) : kKeyMax;
+        }
+#pragma unroll
+        for (uint32_t e = 0; e < 8; ++e) {
+            const uint32_t i = i0 + e * kMergeThreads;
+            if (i < parts * K2) buf[i] = r[e];
+        }
     }
     __syncthreads();
-    for (uint32_t width = 1; width < parts; width <<= 1) {
-        const uint32_t pairs = parts / (2 * width);
-        for (uint32_t i = tid; i < pairs * K2; i += kMergeThreads) {       // the K2 smallest of each pair, into its first list
-            const uint32_t pr = i / K2, j = i - pr * K2;
-            unsigned long long *a = buf + (size_t)pr * 2 * width * K2, *c = a + (size_t)width * K2;
-            const unsigned long long x = a[j], y = c[K2 - 1 - j];
-            a[j] = x < y ? x : y;
-        }
+    bool selected = false;
+    if (parts >= 4) {
+        const uint32_t m = (k + parts - 1) / parts;
+        if (tid < parts) atomicMax(&s_bound, buf[((size_t)tid << lg) + m - 1]);
         __syncthreads();
-        for (uint32_t stride = K2 >> 1; stride > 0; stride >>= 1) {        // bitonic -> ascending
-            for (uint32_t i = tid; i < pairs * (K2 >> 1); i += kMergeThreads) {
-                const uint32_t pr = i / (K2 >> 1), j = i - pr * (K2 >> 1);
-                unsigned long long *a = buf + (size_t)pr * 2 * width * K2;
-                const uint32_t lo = 2 * j - (j & (stride - 1)), hi = lo + stride;
-                const unsigned long long x = a[lo], y = a[hi];
-                if (x > y) { a[lo] = y; a[hi] = x; }
+        const unsigned long long T = s_bound;
+        if (T != kKeyMax) {                                    // every part has at least m keys
+            if (tid < parts) {                                 // keys <= T of part tid: a prefix of its sorted list
+                const unsigned long long *a = buf + ((size_t)tid << lg);
+                uint32_t lo = 0, hi = K2;
+                while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (a[mid] <= T) lo = mid + 1; else hi = mid; }
+                s_off[tid + 1] = lo;
+            }
+            if (tid == 0) s_off[0] = 0;
+            __syncthreads();
+            if (tid == 0) for (uint32_t q = 0; q < parts; ++q) s_off[q + 1] += s_off[q];
+            __syncthreads();
+            const uint32_t total = s_off[parts];
+            if (total <= kMergeSelect) {                       // uniform: gather the prefixes (through registers: in place)
+                unsigned long long r[kMergeSelect / kMergeThreads];
+#pragma unroll
+                for (uint32_t e = 0; e < kMergeSelect / kMergeThreads; ++e) {
+                    const uint32_t i = tid + e * kMergeThreads;
+                    r[e] = kKeyMax;
+                    if (i < total) {
+                        uint32_t q = 0;
+                        while (s_off[q + 1] <= i) ++q;
+                        r[e] = buf[((size_t)q << lg) + (i - s_off[q])];
+                    }
+                }
+                __syncthreads();
+                uint32_t P = 32;
+                while (P < total) P <<= 1;
+#pragma unroll
+                for (uint32_t e = 0; e < kMergeSelect / kMergeThreads; ++e) {
+                    const uint32_t i = tid + e * kMergeThreads;
+                    if (i < P) buf[i] = r[e];
+                }
+                __syncthreads();
+                bitonic_sort_smem(buf, P, 2);
+                selected = true;
+            }
+        }
+    }
+    if (!selected) {
+        for (uint32_t width = 1; width < parts; width <<= 1) {
+            const uint32_t pairs = parts / (2 * width);
+            for (uint32_t i = tid; i < pairs * K2; i += kMergeThreads) {   // the K2 smallest of each pair, into its first list
+                const uint32_t pr = i >> lg, j = i & (K2 - 1);
+                unsigned long long *a = buf + (size_t)pr * 2 * width * K2, *c = a + (size_t)width * K2;
+                const unsigned long long x = a[j], y = c[K2 - 1 - j];
+                a[j] = x < y ? x : y;
             }
             __syncthreads();
+            for (uint32_t stride = K2 >> 1; stride > 0; stride >>= 1) {    // bitonic -> ascending
+                for (uint32_t i = tid; i < pairs * (K2 >> 1); i += kMergeThreads) {
+                    const uint32_t pr = i >> (lg - 1), j = i & ((K2 >> 1) - 1);
+                    unsigned long long *a = buf + (size_t)pr * 2 * width * K2;
+                    const uint32_t lo = 2 * j - (j & (stride - 1)), hi = lo + stride;
+                    const unsigned long long x = a[lo], y = a[hi];
+                    if (x > y) { a[lo] = y; a[hi] = x; }
+                }
+                __syncthreads();
+            }
         }
     }
     const uint32_t U = uniq_counts[b], cnt = U < k ? U : k;
