@@ -51,6 +51,7 @@ struct fann_index {
     uint32_t force_mode = 2;               // dedup placement: 0 ordered, 1 hashed, 2 decided per query (FANN_DEDUP_MODE)
     uint32_t scan_ring = 3;                // scan kernel: stages of the per-warp code-row ring, 0 = rows through registers (FANN_SCAN_RING)
     bool partition = true;                 // split lists into their dedup classes first (FANN_PARTITION=0: filter per pass)
+    bool host_direct = true;               // host entries: kernels write results straight into pinned host output arrays (FANN_HOST_DIRECT=0: staged + copied)
     bool split_scan = true;                // several scan CTAs per query when the batch is smaller than the machine (FANN_SPLIT_SCAN=0: one)
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint32_t dedup_smem_half = 0;          // same for two CTAs per SM
@@ -260,6 +261,7 @@ extern "C" int fann_create(fann_index **out, int device)
     if (const char *s = getenv("FANN_DEDUP_MODE")) { int v = atoi(s); if (v == 0 || v == 1) ix->force_mode = (uint32_t)v; }
     if (const char *s = getenv("FANN_PARTITION")) ix->partition = atoi(s) != 0;
     if (const char *s = getenv("FANN_SPLIT_SCAN")) ix->split_scan = atoi(s) != 0;
+    if (const char *s = getenv("FANN_HOST_DIRECT")) ix->host_direct = atoi(s) != 0;
     if (const char *s = getenv("FANN_LISTS_DIRECT")) ix->lists_direct = atoi(s) != 0;
     if (const char *s = getenv("FANN_SCAN_RING")) { int v = atoi(s); if (v == 0 || v == 3) ix->scan_ring = (uint32_t)v; }
     if (const char *s = getenv("FANN_DEDUP_THREADS")) { int v = atoi(s); if (v == 512 || v == 1024) ix->dedup_threads = (uint32_t)v; }
@@ -720,6 +722,17 @@ extern "C" size_t fann_search_host_scratch_bytes(const fann_index *ix, uint32_t 
     return h.total;
 }
 
+// The device address of a page-locked host array (cudaHostAlloc / cudaHostRegister: what pinned torch tensors are),
+// or NULL for pageable memory.  The host entries hand such output arrays to the kernels themselves: a query's results
+// cross PCIe while the other queries are still being scanned, and no copy follows the last kernel.
+static void *mapped_host_ptr(const void *host)
+{
+    if (!host) return nullptr;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return a.type == cudaMemoryTypeHost ? a.devicePointer : nullptr;
+}
+
 extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t B,
                                 const float *codebooks_d, uint32_t dsub,
                                 const int64_t *cand_offsets_h, const uint32_t *cand_ids_h,
@@ -751,6 +764,16 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
     Geom g;
     geometry(ix, k, B, total, &g);                             // one dedup CTA shape for all chunks: the layout depends on it
     const uint32_t nchunk = (B >= 64 && total >= (4u << 20) && ix->chunks == 1) ? 8u : 1u;   // 16 MB of IDs and up
+    uint32_t *o_ids = (uint32_t *)(s + h.out_ids), *o_counts = (uint32_t *)(s + h.out_counts);
+    float *o_dists = (float *)(s + h.out_dists);
+    bool direct = false;
+    if (ix->host_direct) {
+        void *di = mapped_host_ptr(out_ids_h), *dd = mapped_host_ptr(out_dists_h), *dc = mapped_host_ptr(out_counts_h);
+        if (di && dd && (dc || !out_counts_h)) {
+            direct = true; o_ids = (uint32_t *)di; o_dists = (float *)dd;
+            if (dc) o_counts = (uint32_t *)dc;
+        }
+    }
     CtxLease lease(ix);
     CallCtx *cx = lease.c;
     if (!cx) return fail(FANN_ECUDA, "fann_search_host: could not create the transfer stream");
@@ -765,15 +788,16 @@ extern "C" int fann_search_host(fann_index *ix, const float *queries_h, uint32_t
         CUDA_TRY(cudaStreamWaitEvent(stream, cx->ev_done[c], 0));
         rc = run_path(ix, false, (const float *)(s + h.lut) + (size_t)b0 * ix->M * 256, b1 - b0,
                       (const int64_t *)(s + h.offsets) + b0, (const uint32_t *)(s + h.ids), total, k,
-                      (uint32_t *)(s + h.out_ids) + (size_t)b0 * k, (float *)(s + h.out_dists) + (size_t)b0 * k,
-                      (uint32_t *)(s + h.out_counts) + b0, nullptr, nullptr, nullptr,
+                      o_ids + (size_t)b0 * k, o_dists + (size_t)b0 * k, o_counts + b0, nullptr, nullptr, nullptr,
                       s + h.ws, h.ws_bytes, stream, g.dedup_threads, c > 0, nchunk == 1, nchunk == 1);
         if (rc != FANN_OK) return rc;
     }
-    CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
-    CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
-    if (out_counts_h)
-        CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
+    if (!direct) {
+        CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+        CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+        if (out_counts_h)
+            CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
+    }
     CUDA_TRY(cudaStreamSynchronize(stream));
     return fann_workspace_status(ix, s + h.ws, stream);
 }
@@ -1003,14 +1027,25 @@ extern "C" int fann_search_lists_host(fann_index *ix, const float *queries_h, ui
     // ramp-up and drain, 4.1 ms over the device path, than the overlap saves, 2.9 ms in one piece.)
     ListsLayout l;
     lists_layout(ix, B, max_total_cands, k, &l);
+    uint32_t *o_ids = (uint32_t *)(s + h.out_ids), *o_counts = (uint32_t *)(s + h.out_counts);
+    float *o_dists = (float *)(s + h.out_dists);
+    bool direct = false;
+    if (ix->host_direct) {                                     // pinned output arrays: the kernels write them (80 MB, 1.4 ms of copies at u8_1b_m64)
+        void *di = mapped_host_ptr(out_ids_h), *dd = mapped_host_ptr(out_dists_h), *dc = mapped_host_ptr(out_counts_h);
+        if (di && dd && (dc || !out_counts_h)) {
+            direct = true; o_ids = (uint32_t *)di; o_dists = (float *)dd;
+            if (dc) o_counts = (uint32_t *)dc;
+        }
+    }
     rc = search_lists_impl(ix, (const float *)(s + h.lut), B, (const uint32_t *)(s + h.probes), nprobe, max_total_cands, k,
-                           (uint32_t *)(s + h.out_ids), (float *)(s + h.out_dists), (uint32_t *)(s + h.out_counts), nullptr,
-                           s + h.ws, l, stream);
+                           o_ids, o_dists, o_counts, nullptr, s + h.ws, l, stream);
     if (rc != FANN_OK) return rc;
-    CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
-    CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
-    if (out_counts_h)
-        CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
+    if (!direct) {
+        CUDA_TRY(cudaMemcpyAsync(out_ids_h, s + h.out_ids, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+        CUDA_TRY(cudaMemcpyAsync(out_dists_h, s + h.out_dists, (size_t)B * k * 4, cudaMemcpyDeviceToHost, stream));
+        if (out_counts_h)
+            CUDA_TRY(cudaMemcpyAsync(out_counts_h, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream));
+    }
     return fann_search_lists_status(ix, s + h.ws, B, max_total_cands, k, nullptr, stream);   // synchronises
 }
 
@@ -1315,6 +1350,9 @@ extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const fl
     for (auto &g : cache)
         if (g.B == B && g.nprobe == nprobe && g.k == k && g.codebooks == codebooks_d) exec = g.exec;
     if (!exec) {
+        // results: written by the kernels straight into the block's pinned staging buffer (its device address)
+        char *o = ix->host_direct ? (char *)mapped_host_ptr(st) : nullptr;
+        const bool direct = o != nullptr;
         CUDA_TRY(cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal));
         int rc = FANN_OK;
         cudaError_t ce = cudaMemcpyAsync(s + h.queries, st + pool->st_queries, qbytes, cudaMemcpyHostToDevice, stream);
@@ -1322,11 +1360,15 @@ extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const fl
         if (ce == cudaSuccess) rc = fann_build_lut(ix, (const float *)(s + h.queries), B, codebooks_d, dsub, (float *)(s + h.lut), stream);
         if (ce == cudaSuccess && rc == FANN_OK)
             rc = search_lists_impl(ix, (const float *)(s + h.lut), B, (const uint32_t *)(s + h.probes), nprobe, pool->max_cands, k,
-                                   (uint32_t *)(s + h.out_ids), (float *)(s + h.out_dists), (uint32_t *)(s + h.out_counts), nullptr,
+                                   direct ? (uint32_t *)(o + pool->st_ids) : (uint32_t *)(s + h.out_ids),
+                                   direct ? (float *)(o + pool->st_dists) : (float *)(s + h.out_dists),
+                                   direct ? (uint32_t *)(o + pool->st_counts) : (uint32_t *)(s + h.out_counts), nullptr,
                                    s + h.ws, l, stream);
-        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_ids, s + h.out_ids, obytes, cudaMemcpyDeviceToHost, stream);
-        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_dists, s + h.out_dists, obytes, cudaMemcpyDeviceToHost, stream);
-        if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_counts, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream);
+        if (!direct) {
+            if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_ids, s + h.out_ids, obytes, cudaMemcpyDeviceToHost, stream);
+            if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_dists, s + h.out_dists, obytes, cudaMemcpyDeviceToHost, stream);
+            if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_counts, s + h.out_counts, (size_t)B * 4, cudaMemcpyDeviceToHost, stream);
+        }
         if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_hdr, s + h.ws + l.hdr, sizeof(ListsHeader), cudaMemcpyDeviceToHost, stream);
         if (ce == cudaSuccess) ce = cudaMemcpyAsync(st + pool->st_hdr + sizeof(ListsHeader), s + h.ws + l.ws, sizeof(WsHeader), cudaMemcpyDeviceToHost, stream);
         cudaGraph_t graph = nullptr;

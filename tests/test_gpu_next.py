@@ -122,7 +122,12 @@ def test_search_lists_padding_unknown_lists_and_capacity(fann, wl_int, monkeypat
     assert err.value.code == -5 and err.value.total_cands == need
 
 
-def test_search_lists_host_entry(fann, wl_int):
+@pytest.mark.parametrize("outputs", ["pinned", "pageable", "pinned_copied"])
+def test_search_lists_host_entry(fann, wl_int, monkeypatch, outputs):
+    """Pinned output arrays are written by the kernels themselves, pageable ones through a staged copy
+    (FANN_HOST_DIRECT=0: always the copy): the same bytes."""
+    if outputs == "pinned_copied":
+        monkeypatch.setenv("FANN_HOST_DIRECT", "0")
     w = wl_int
     ix, res = _search_lists(fann, w, w.probes.numpy().view(np.uint32))
     B, k, nprobe = w.cfg.B, w.cfg.k, w.cfg.nprobe
@@ -130,9 +135,11 @@ def test_search_lists_host_entry(fann, wl_int):
     need = fann.fann_search_lists_host_scratch_bytes(ix.handle, B, w.cfg.dsub, nprobe, cap, k)
     scratch = torch.empty(need, dtype=torch.uint8, device=DEV)
     q_h, p_h = w.queries.pin_memory(), w.probes.contiguous().pin_memory()
-    oi = torch.empty((B, k), dtype=torch.int32).pin_memory()
-    od = torch.empty((B, k), dtype=torch.float32).pin_memory()
-    oc = torch.empty(B, dtype=torch.int32).pin_memory()
+    oi = torch.empty((B, k), dtype=torch.int32)
+    od = torch.empty((B, k), dtype=torch.float32)
+    oc = torch.empty(B, dtype=torch.int32)
+    if outputs != "pageable":
+        oi, od, oc = oi.pin_memory(), od.pin_memory(), oc.pin_memory()
     for _ in range(2):
         oi.fill_(0)
         fann.fann_search_lists_host(ix.handle, q_h, B, w.codebooks.to(DEV), w.cfg.dsub, p_h, nprobe, cap, k, oi, od, oc,

@@ -441,16 +441,20 @@ def test_argument_errors(fann, tiny):
         ix.load_codes(w.codes[:10, :8].contiguous().to(DEV))                    # M changed
 
 
-def test_host_entry_matches_device_entry(fann, w_i8):
+@pytest.mark.parametrize("outputs", ["pinned", "pageable"])
+def test_host_entry_matches_device_entry(fann, w_i8, outputs):
+    """Pinned host outputs are written by the kernels directly, pageable ones by a copy after them."""
     w = w_i8
     ix, _, res = gpu_search(fann, w)
     B, k, total = w.cfg.B, w.cfg.k, w.cand_ids.numel()
     need = fann.fann_search_host_scratch_bytes(ix.handle, B, w.cfg.dsub, total, k)
     scratch = torch.empty(need, dtype=torch.uint8, device=DEV)
     q_h, off_h, ids_h = w.queries.pin_memory(), w.cand_offsets.pin_memory(), w.cand_ids.pin_memory()
-    oi = torch.empty((B, k), dtype=torch.int32).pin_memory()
-    od = torch.empty((B, k), dtype=torch.float32).pin_memory()
-    oc = torch.empty(B, dtype=torch.int32).pin_memory()
+    oi = torch.empty((B, k), dtype=torch.int32)
+    od = torch.empty((B, k), dtype=torch.float32)
+    oc = torch.empty(B, dtype=torch.int32)
+    if outputs == "pinned":
+        oi, od, oc = oi.pin_memory(), od.pin_memory(), oc.pin_memory()
     fann.fann_search_host(ix.handle, q_h, B, w.codebooks.to(DEV), w.cfg.dsub, off_h, ids_h, k, oi, od, oc,
                           scratch, need, torch.cuda.current_stream().cuda_stream)
     assert np.array_equal(oi.numpy().view(np.uint32), res[0])
