@@ -187,6 +187,11 @@ int fann_workspace_modes(fann_index *ix, const void *workspace, uint32_t B, uint
  * (queries are independent), so the transfer and the kernels overlap.
  * queries_h, cand_offsets_h, cand_ids_h, out_*_h: host pointers (pinned memory
  * gives asynchronous copies); layouts as above.  out_counts_h may be NULL.
+ * Output arrays that are all page-locked (cudaHostAlloc / cudaHostRegister) are
+ * written by the kernels themselves through their device address -- a query's
+ * results cross PCIe while other queries are still scanned and no copy follows
+ * the last kernel; they are valid when the call returns, like copied ones.
+ * Pageable arrays (or FANN_HOST_DIRECT=0) take a staged device->host copy.
  * device_scratch: device, >= fann_search_host_scratch_bytes(...), 256-byte aligned.
  */
 size_t fann_search_host_scratch_bytes(const fann_index *ix, uint32_t B, uint32_t dsub,
@@ -252,7 +257,8 @@ int fann_search_lists_status(fann_index *ix, const void *workspace, uint32_t B, 
 /*
  * The same from HOST buffers: query vectors and probes go up (B * (4 d + 4 nprobe) bytes),
  * ids / dists / counts come back; synchronises `stream` and returns the batch's status.
- * queries_h, probes_h, out_*_h: host pointers (pinned memory gives asynchronous copies).
+ * queries_h, probes_h, out_*_h: host pointers (pinned memory gives asynchronous copies;
+ * page-locked output arrays are written by the kernels directly, as in fann_search_host).
  */
 size_t fann_search_lists_host_scratch_bytes(const fann_index *ix, uint32_t B, uint32_t dsub, uint32_t nprobe,
                                             uint64_t max_total_cands, uint32_t k);
@@ -308,7 +314,8 @@ int fann_search_lists_stream_status(fann_index *ix, const void *workspace, uint6
  * the same bytes as the batched entry points give.  fann_search_small_lists replays ONE CUDA
  * graph per call (captured per block and call shape -- B, nprobe, k, codebooks -- on first use):
  * the inputs are copied into the block's pinned staging buffer, the graph copies them up, runs
- * the ten kernels and copies results and status back (FANN_SMALL_GRAPH=0: plain launches).
+ * the kernels -- which write the results straight into the staging buffer -- and copies the
+ * status back (FANN_SMALL_GRAPH=0: plain launches).
  * Errors: EINVAL (NULL, a pool of another index, B / k / dsub / nprobe outside what the pool
  * was created for), EWORKSPACE (more candidate IDs than a block holds), and what the batched
  * entry points return.

@@ -1391,12 +1391,16 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const ScanParams p)
     const uint32_t margin = kScanWarps * 32 * (D ? NBS : NB) + 64;   // keys appended between the buffer passing its limit and the prune
     const uint32_t limit = p.cap - margin;
 
+    // The next work item is taken while the current one is scanned: thread 0 holds the counter's answer in a register
+    // (the atomic's round trip overlaps the scan) and publishes it when the query is done.
+    uint32_t next_work = 0;
+    if (tid == 0) next_work = atomicAdd(p.counter, 1u);
     for (;;) {
-        __syncthreads();                                       // previous query fully done
-        if (tid == 0) misc[2] = atomicAdd(p.counter, 1u);
-        __syncthreads();
+        if (tid == 0) misc[2] = next_work;
+        __syncthreads();                                       // previous query fully done; misc[2] visible
         const uint32_t work = misc[2];                         // (query, part of its distinct list)
         if (work >= (p.q_end - p.q_begin) * p.parts) break;
+        if (tid == 0) next_work = atomicAdd(p.counter, 1u);
         const uint32_t b = p.q_begin + work / p.parts, part = work % p.parts;
         const long long off0 = p.cand_offsets[b];
         uint32_t U = p.uniq_counts[b];
