@@ -141,6 +141,7 @@ struct Geom {
     uint32_t cap, scan_smem, ring;                   // scan: candidate-buffer keys, shared memory per CTA, ring depth
     uint32_t parts, k;                               // scan CTAs per query (> 1 for batches smaller than the machine), k
     uint32_t part_ctas;                              // partition CTAs per query (> 1 for small batches)
+    uint32_t min_classes;                            // lists-direct: at least this many ID-range classes per query (small batches)
 };
 
 // Dedup CTA shape: one 1024-thread CTA per SM with the whole shared memory as its table, or -- when the mean candidate
@@ -173,6 +174,11 @@ static void geometry(const fann_index *ix, uint32_t k, uint32_t B, uint64_t tota
     g->part_ctas = 1;
     if (ix->split_scan && allow_split)
         while (g->part_ctas < 16 && 2 * g->part_ctas * B <= (uint32_t)ix->num_sms) g->part_ctas <<= 1;
+    // lists-direct, small batch: more (smaller) ID-range classes per query than its size asks for, so that one query's
+    // dedup spreads over the machine like its scan does (a class is a run of the 64 grid cells: a power of two)
+    g->min_classes = 1;
+    if (ld && ix->split_scan && allow_split)
+        while (g->min_classes < 32 && g->min_classes * B <= (uint32_t)ix->num_sms) g->min_classes <<= 1;
     g->cap = (k <= 256 || g->ring) ? 4096u : 8192u;            // the ring takes the shared memory of the larger buffer
     g->scan_smem = (uint32_t)scan_smem_bytes(g->cap, g->ring);
 }
@@ -184,7 +190,8 @@ struct WsLayout {
 
 static void ws_layout(uint32_t B, uint64_t total_cands, const Geom &g, bool with_uniq, WsLayout *w)
 {
-    const uint64_t max_items = 2 * ((uint64_t)B + total_cands / g.cap_c + 1);   // x2: the lists-direct path rounds S_b up to a power of two
+    const uint64_t max_items = 2 * ((uint64_t)B + total_cands / g.cap_c + 1) +  // x2: the lists-direct path rounds S_b up to a power of two
+                               (uint64_t)B * (g.min_classes > 1 ? g.min_classes : 0u);
     w->max_items = (uint32_t)(max_items > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : max_items);
     size_t o = 0;
     w->hdr = o;         o = align_up(o + 256, 256);
@@ -505,7 +512,7 @@ static int run_path(fann_index *ix, bool dump, const float *lut, uint32_t B,
                                         item_start, items, uniq_counts, keep_status ? 1u : 0u,
                                         (unsigned long long)total_cands, exact_total ? 1u : 0u,
                                         g.part_ctas > 1 && !ld ? (uint32_t *)(ws + w.bucket_cnt) : nullptr,
-                                        g.part_ctas > 1 && !ld ? (uint32_t *)(ws + w.part_aux) : nullptr, ld ? 1u : 0u);
+                                        g.part_ctas > 1 && !ld ? (uint32_t *)(ws + w.part_aux) : nullptr, ld ? g.min_classes : 0u);
     if (ld)
         lists_classes_kernel<<<B, 256, 0, stream>>>(ix->list_grid, ix->n_lists, ix->N, probes, nprobe, S, item_start,
                                                     (uint32_t)((uint64_t)g.nslots_max * 9 / 10), ix->force_mode, mode,

@@ -289,8 +289,8 @@ __global__ void plan_kernel(const long long *__restrict__ cand_offsets, uint32_t
             if (c < 0) c = 0;
             s = (uint32_t)((c + cap_c - 1) / cap_c);
             if (s == 0) s = 1;
-            if (pow2_classes && s <= kGridCells) {             // lists-direct: ID-range classes are runs of grid cells
-                uint32_t s2 = 1;
+            if (pow2_classes && s <= kGridCells) {             // lists-direct: ID-range classes are runs of grid cells,
+                uint32_t s2 = pow2_classes < kGridCells ? pow2_classes : kGridCells;   // at least pow2_classes of them
                 while (s2 < s) s2 <<= 1;
                 s = s2;
             }
