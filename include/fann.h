@@ -143,6 +143,41 @@ int fann_dedup_scan_topk(fann_index *ix, const float *lut, uint32_t B,
                          void *workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * The same call for callers that cannot allocate device memory (code under CUDA
+ * graph capture, serving loops and harnesses that forbid cudaMalloc): steps (5)-(7),
+ * PAPER.md:L127-L133, with the workspace in a file-scope device array of the library
+ * instead of a caller's allocation.  The call allocates nothing -- no cudaMalloc, no
+ * cudaFree, no stream or event creation -- and enqueues on `stream` only: one
+ * 256-byte memset (the workspace header: status word and work counters start at
+ * zero), the kernels of fann_dedup_scan_topk, and a 4-byte device-to-device copy of
+ * the status word.  Arguments, layouts and results as fann_dedup_scan_topk, plus
+ * out_status  device, 1 uint32 (may be NULL): what fann_workspace_status would have
+ *             reported, valid once `stream` has run the call -- 0 = results valid,
+ *             FANN_STATUS_TABLE_FULL / FANN_STATUS_BAD_TOTAL bits otherwise.
+ * Limit: the batch must need at most FANN_STATIC_WS_BYTES (32 MiB) of workspace, i.e.
+ * fann_workspace_bytes(ix, B, total_cands, k) <= FANN_STATIC_WS_BYTES -- about 2.7 M
+ * candidate IDs per call (20 queries of 128 k IDs, 80 of 32 k).  A larger batch is
+ * refused with FANN_EWORKSPACE and a message naming both sizes; nothing is enqueued.
+ * The array is ONE per device for the whole process (every GPU that loads the library
+ * holds its 32 MiB until exit), shared by every handle and every call and keeping the
+ * last call's contents: calls of this entry that overlap on the GPU -- two streams,
+ * two host threads, two handles on one device -- race on it and give wrong results;
+ * serialise them (one stream, or events).  It does not conflict with the entry points
+ * that take a caller's workspace.  Its device address is resolved once per device in
+ * fann_create; FANN_ECUDA if that failed; FANN_EUNSUPPORTED with FANN_CHUNKS > 1 (the
+ * chunked path creates a stream).
+ */
+#define FANN_STATIC_WS_BYTES (32u * 1024u * 1024u)
+#define FANN_STATUS_TABLE_FULL 1u   /* a dedup table filled up: FANN_EOVERFLOW of fann_workspace_status */
+#define FANN_STATUS_BAD_TOTAL  2u   /* total_cands disagrees with cand_offsets: its FANN_EINVAL         */
+int fann_dedup_scan_topk_static(fann_index *ix, const float *lut, uint32_t B,
+                                const int64_t *cand_offsets, const uint32_t *cand_ids,
+                                uint64_t total_cands, uint32_t k,
+                                uint32_t *out_ids, float *out_dists,
+                                uint32_t *out_counts, uint32_t *out_uniq,
+                                uint32_t *out_status, void *stream);
+
+/*
  * Step (5) alone, through the same kernel and hash tables as the call above
  * (test hook for the bit-exact dedup check): the distinct valid IDs of query b,
  * in any order, are written to uniq_ids[cand_offsets[b] .. +uniq_counts[b]).

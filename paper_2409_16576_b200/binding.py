@@ -22,6 +22,8 @@ FANN_MAX_K = 1024
 FANN_MAX_NPROBE = 8192
 FANN_ELEM_F32, FANN_ELEM_U8, FANN_ELEM_I8 = 0, 1, 2
 FANN_OK = 0
+FANN_STATIC_WS_BYTES = 32 * 1024 * 1024      # fann_dedup_scan_topk_static: the static workspace (fann.h)
+FANN_STATUS_TABLE_FULL, FANN_STATUS_BAD_TOTAL = 1, 2
 
 _lib = None
 
@@ -69,6 +71,7 @@ def load_library():
         "fann_build_lut": (i, [p, p, u32, p, u32, p, p]),
         "fann_workspace_bytes": (sz, [p, u32, u64, u32]),
         "fann_dedup_scan_topk": (i, [p, p, u32, p, p, u64, u32, p, p, p, p, p, sz, p]),
+        "fann_dedup_scan_topk_static": (i, [p, p, u32, p, p, u64, u32, p, p, p, p, p, p]),
         "fann_dedup_only": (i, [p, u32, p, p, u64, p, p, p, sz, p]),
         "fann_workspace_status": (i, [p, p, p]),
         "fann_workspace_modes": (i, [p, p, u32, u64, u32, C.POINTER(u32), C.POINTER(u32), p]),
@@ -163,6 +166,14 @@ def fann_dedup_scan_topk(ix, lut, B, cand_offsets, cand_ids, total_cands, k, out
                                                total_cands, k, _addr(out_ids), _addr(out_dists),
                                                _addr(out_counts), _addr(out_uniq), _addr(workspace),
                                                workspace_bytes, stream))
+
+
+def fann_dedup_scan_topk_static(ix, lut, B, cand_offsets, cand_ids, total_cands, k, out_ids, out_dists,
+                                out_counts, out_uniq, out_status, stream=None) -> None:
+    """No allocation anywhere: the workspace is a device array of the library (FANN_STATIC_WS_BYTES)."""
+    _check(load_library().fann_dedup_scan_topk_static(ix, _addr(lut), B, _addr(cand_offsets), _addr(cand_ids),
+                                                      total_cands, k, _addr(out_ids), _addr(out_dists),
+                                                      _addr(out_counts), _addr(out_uniq), _addr(out_status), stream))
 
 
 def fann_dedup_only(ix, B, cand_offsets, cand_ids, total_cands, uniq_ids, uniq_counts, workspace,

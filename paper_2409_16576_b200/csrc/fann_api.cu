@@ -56,6 +56,8 @@ struct fann_index {
     uint32_t dedup_smem = 0;               // dynamic shared memory of a dedup CTA
     uint32_t dedup_smem_half = 0;          // same for two CTAs per SM
     uint32_t dedup_threads = 0;            // 0: chosen per call (geometry()); 1024 or 512: forced (FANN_DEDUP_THREADS)
+    void *static_ws = nullptr;             // device address of g_static_ws on this device (fann_dedup_scan_topk_static), resolved in fann_create
+    cudaError_t static_ws_err = cudaSuccess;
     std::atomic<uint64_t> launches{0};
     std::atomic<uint32_t> generation{0};   // bumped by the loaders: captured graphs (fann_pool) hold the arrays' addresses
     // everything below is shared by concurrent callers and guarded by `mu`
@@ -133,6 +135,33 @@ struct CtxLease {
         ix->ctx_pool.push_back(c);
     }
 };
+
+// ---------------------------------------------------------------- the no-allocation entry's workspace
+
+// fann_dedup_scan_topk_static: the workspace of the path as a file-scope device array (fann.h).  In host code the
+// name g_static_ws is a host-side stand-in of the symbol, NOT a device address: the address the kernels get comes
+// from cudaGetSymbolAddress, asked once per device with that device current (fann_create) and kept here.
+static __device__ __align__(256) unsigned char g_static_ws[FANN_STATIC_WS_BYTES];
+
+constexpr int kMaxDevices = 64;
+static std::mutex g_static_mu;
+static void *g_static_ptr[kMaxDevices] = {};
+
+// The calling thread's current device must be `device`.
+static cudaError_t static_ws_resolve(int device, void **out)
+{
+    *out = nullptr;
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[device]) {
+        void *ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_static_ws);
+        if (e != cudaSuccess) return e;
+        g_static_ptr[device] = ptr;
+    }
+    *out = g_static_ptr[device];
+    return cudaSuccess;
+}
 
 // ---------------------------------------------------------------- geometry + workspace layout
 
@@ -260,6 +289,8 @@ extern "C" int fann_create(fann_index **out, int device)
     CUDA_TRY(cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device));
     fann_index *ix = new fann_index();
     ix->device = device; ix->num_sms = num_sms; ix->smem_optin = smem_optin;
+    ix->static_ws_err = static_ws_resolve(device, &ix->static_ws);     // `device` is current (guard above)
+    if (ix->static_ws_err != cudaSuccess) cudaGetLastError();          // only fann_dedup_scan_topk_static needs it: it reports
     ix->dedup_smem = (uint32_t)smem_optin;
     // two dedup CTAs per SM: each gets half of the SM's shared memory less the 1 KB the driver reserves per CTA
     ix->dedup_smem_half = (uint32_t)((per_sm / 2 - 1024) & ~255);
@@ -643,6 +674,48 @@ extern "C" int fann_dedup_scan_topk(fann_index *ix, const float *lut, uint32_t B
     if (k == 0 || k > FANN_MAX_K) return fail(FANN_EUNSUPPORTED, "fann_dedup_scan_topk: k=%u not in 1..%u", k, FANN_MAX_K);
     return run_path(ix, false, lut, B, cand_offsets, cand_ids, total_cands, k, out_ids, out_dists,
                     out_counts, out_uniq, nullptr, nullptr, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+// The same path with its workspace in g_static_ws: allocates nothing (fann.h).  One array per device, shared by
+// every call: overlapping calls race.
+extern "C" int fann_dedup_scan_topk_static(fann_index *ix, const float *lut, uint32_t B,
+                                           const int64_t *cand_offsets, const uint32_t *cand_ids,
+                                           uint64_t total_cands, uint32_t k,
+                                           uint32_t *out_ids, float *out_dists,
+                                           uint32_t *out_counts, uint32_t *out_uniq,
+                                           uint32_t *out_status, void *stream_)
+{
+    if (!ix || !lut || !cand_offsets || !out_ids || !out_dists)
+        return fail(FANN_EINVAL, "fann_dedup_scan_topk_static: NULL argument");
+    if (!cand_ids && total_cands) return fail(FANN_EINVAL, "fann_dedup_scan_topk_static: cand_ids is NULL");
+    if (!ix->codes) return fail(FANN_EINVAL, "fann_dedup_scan_topk_static: load codes first");
+    if (B == 0) return fail(FANN_EINVAL, "fann_dedup_scan_topk_static: B == 0");
+    if (k == 0 || k > FANN_MAX_K)
+        return fail(FANN_EUNSUPPORTED, "fann_dedup_scan_topk_static: k=%u not in 1..%u", k, FANN_MAX_K);
+    if (((uintptr_t)out_status & 3) != 0) return fail(FANN_EINVAL, "fann_dedup_scan_topk_static: out_status must be 4-byte aligned");
+    if (!ix->static_ws)
+        return fail(FANN_ECUDA, "fann_dedup_scan_topk_static: cudaGetSymbolAddress of the static workspace failed in fann_create: %s",
+                    cudaGetErrorString(ix->static_ws_err));
+    if (ix->chunks != 1)
+        return fail(FANN_EUNSUPPORTED, "fann_dedup_scan_topk_static: not with FANN_CHUNKS > 1 (the chunked path creates a stream)");
+    Geom g;
+    geometry(ix, k, B, total_cands, &g);                       // as run_path and fann_workspace_bytes compute it
+    WsLayout w;
+    ws_layout(B, total_cands, g, true, &w);
+    if (w.total > (size_t)FANN_STATIC_WS_BYTES)
+        return fail(FANN_EWORKSPACE, "fann_dedup_scan_topk_static: B=%u, total_cands=%llu, k=%u need %zu bytes of workspace, "
+                    "the static array holds %u (FANN_STATIC_WS_BYTES); use fann_dedup_scan_topk with a workspace of your own",
+                    B, (unsigned long long)total_cands, k, w.total, (unsigned)FANN_STATIC_WS_BYTES);
+    DeviceGuard guard(ix->device);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    // the array keeps the last call's contents: the header (status word, work counters) starts at zero
+    CUDA_TRY(cudaMemsetAsync((char *)ix->static_ws + w.hdr, 0, 256, stream));
+    const int rc = run_path(ix, false, lut, B, cand_offsets, cand_ids, total_cands, k, out_ids, out_dists,
+                            out_counts, out_uniq, nullptr, nullptr, ix->static_ws, (size_t)FANN_STATIC_WS_BYTES, stream);
+    if (rc != FANN_OK) return rc;
+    if (out_status)
+        CUDA_TRY(cudaMemcpyAsync(out_status, (const char *)ix->static_ws + w.hdr, 4, cudaMemcpyDeviceToDevice, stream));
+    return FANN_OK;
 }
 
 extern "C" int fann_dedup_only(fann_index *ix, uint32_t B, const int64_t *cand_offsets,
