@@ -88,6 +88,34 @@ def test_split_scan_edge_lists(fann):
     ix.close()
 
 
+@pytest.mark.parametrize("B", [1, 9, 20, 40])
+def test_split_scan_distance_follows_the_id(fann, B):
+    """The slices of a query's distinct list are ID ranges (ordered dedup placement).  Here the distance is a monotone
+    function of the ID with 780 equal distances in a row, so the top-k sits in ONE slice (the lowest IDs for query 0,
+    the highest for query 1, the middle for query 2): the merge's bound from the parts' m-th keys is then far above
+    the k-th key, its selection does not apply and it falls back to merging the parts pairwise; ties are decided by ID
+    across slice borders.  16, 16, 4 and 2 scan CTAs per query."""
+    rng = np.random.default_rng(11)
+    N, M, dsub = 200_000, 16, 4
+    codes = np.repeat((np.arange(N, dtype=np.int64) * 256 // N).astype(np.uint8)[:, None], M, axis=1)
+    cb = np.repeat(np.arange(256, dtype=np.float32)[None, :, None], M, axis=0).repeat(dsub, axis=2)   # centroid j = (j, j, j, j)
+    q = np.zeros((B, M * dsub), dtype=np.float32)
+    q[1::3] = 255.0
+    q[2::3] = 128.0
+    lists = [rng.integers(0, N, 60_000 + 1000 * b).astype(np.uint32) for b in range(B)]
+    off = np.zeros(B + 1, np.int64)
+    off[1:] = np.cumsum([len(x) for x in lists])
+    ids = np.concatenate(lists)
+    ix = fann.FannIndex(0)
+    ix.load_codes(torch.from_numpy(codes).to(DEV))
+    lut = ix.build_lut(torch.from_numpy(q).to(DEV), torch.from_numpy(cb).to(DEV))
+    for k in (1000, 64, 1):
+        o = ix.dedup_scan_topk(lut, torch.from_numpy(off).to(DEV), torch.from_numpy(ids.view(np.int32)).to(DEV), k, check=True)
+        torch.cuda.synchronize()
+        check_exact((np_u32(o[0]), o[1].cpu().numpy(), np_u32(o[2]), np_u32(o[3])), oracle.search(q, cb, codes, off, ids, k))
+    ix.close()
+
+
 def test_split_scan_fp32_band(fann):
     w = make_workload(CONFIGS["tiny_local"])
     ix = fann.FannIndex(0)
