@@ -1313,8 +1313,9 @@ extern "C" int fann_pool_create(fann_index *ix, uint32_t n_blocks, uint32_t max_
         lists_host_layout(ix, max_B, dsub, max_nprobe, max_cands, k_max, &lh);
         if (lh.total > need) need = lh.total;
     }
-    // the partial top-k of the scan parts depends on the batch size of the call: at most num_sms x k keys
-    need = align_up(need + (size_t)ix->num_sms * k_max * 8 + 4096, 256);
+    // what depends on the batch size of the call and is not largest at max_B: the partial top-k of the scan parts (at
+    // most num_sms x k keys) and the extra dedup items of a small lists-direct batch (at most 2 num_sms, 12 bytes each)
+    need = align_up(need + (size_t)ix->num_sms * k_max * 8 + (size_t)2 * ix->num_sms * 12 + 8192, 256);
     fann_pool *p = new fann_pool();
     p->ix = ix; p->block_bytes = need; p->n_blocks = n_blocks; p->max_B = max_B; p->k_max = k_max; p->dsub = dsub;
     p->max_nprobe = max_nprobe; p->max_cands = max_cands;
@@ -1418,6 +1419,8 @@ extern "C" int fann_search_small_lists(fann_index *ix, fann_pool *pool, const fl
     memcpy(st + pool->st_probes, probes_h, pbytes);
     ListsHostScratch h;
     lists_host_layout(ix, B, dsub, nprobe, pool->max_cands, k, &h);
+    if (h.total > pool->block_bytes)
+        return fail(FANN_EWORKSPACE, "fann_search_small_lists: the call needs %zu bytes, a block of the pool has %zu", h.total, pool->block_bytes);
     ListsLayout l;
     lists_layout(ix, B, pool->max_cands, k, &l);
     cudaGraphExec_t exec = nullptr;

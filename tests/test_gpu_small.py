@@ -187,6 +187,34 @@ def test_pool_entries_match_the_oracle(fann, wl, ref, monkeypatch, graphs):
     ix.close()
 
 
+def test_pool_block_holds_every_batch_size_up_to_max_b(fann, wl, ref):
+    """The workspace of a call is not largest at max_B: small batches take several scan CTAs per query (partial top-k
+    lists) and up to 32 dedup classes per query.  A pool created for max_B must serve every B <= max_B, through both
+    forms, with the oracle's bytes."""
+    w = wl
+    ix = fann.FannIndex(0)
+    ix.load_codes(w.codes.to(DEV))
+    ix.load_lists(w.list_offsets.to(DEV), w.list_ids.to(DEV))
+    max_B = w.cfg.B
+    pool = _pool(fann, ix, w, 1, max_B)
+    cb = w.codebooks.to(DEV)
+    k = w.cfg.k
+    for B in list(range(1, 12)) + [16, 18, 19, 24, 30, 37, 38, max_B]:
+        q, off, ids = _sub(w, 0, B)
+        P = np.ascontiguousarray(w.probes[:B].numpy())
+        r = _ref_rows(ref, 0, B)
+        for form in ("lists", "ids"):
+            oi, od, oc = np.zeros((B, k), np.uint32), np.zeros((B, k), np.float32), np.zeros(B, np.uint32)
+            if form == "lists":
+                fann.fann_search_small_lists(ix.handle, pool, q.numpy(), B, cb, w.cfg.dsub, P, w.cfg.nprobe, k, oi, od, oc)
+            else:
+                fann.fann_search_small(ix.handle, pool, q.numpy(), B, cb, w.cfg.dsub, off.numpy(), ids.numpy(), k, oi, od, oc)
+            assert np.array_equal(oi, r["ids"]) and np.array_equal(od.view(np.uint32), r["dists"].view(np.uint32)), (B, form)
+            assert np.array_equal(oc, r["counts"])
+    fann.fann_pool_destroy(pool)
+    ix.close()
+
+
 def test_concurrent_host_threads_one_handle(fann, wl, ref):
     """PAPER.md:L204 "each CPU thread handles an individual query": 8 host threads, one handle, a pool of 3 blocks
     (so calls also wait for a block), every query answered once through both entry forms; the bytes are the
