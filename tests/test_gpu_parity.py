@@ -419,6 +419,57 @@ def test_edge_cases(fann, w_int):
             assert np.array_equal(res[0][a], res[0][b]) and np.array_equal(res[1][a], res[1][b])
 
 
+@pytest.mark.parametrize("seed", range(40))
+def test_random_shapes_differential(fann, seed):
+    """Differential test on random problem shapes nobody chose: M, dsub, N, batch size (also below half the SMs: several
+    scan CTAs per query), list lengths from 0 to 150 k with a random share of repeats, invalid IDs sprinkled in, k from
+    1 to 1024, IDs either spread over [0, N) or bunched.  Integer data, so the oracle's bytes are the bar; the lookup
+    table is checked too."""
+    rng = np.random.default_rng(1000 + seed)
+    M = int(rng.choice([1, 3, 8, 16, 17, 25, 32, 33, 48, 64]))
+    dsub = int(rng.choice([1, 2, 4, 8]))
+    N = int(rng.choice([300, 5_000, 70_000, 400_000]))
+    B = int(rng.choice([1, 2, 5, 13, 40, 75, 150, 300]))
+    k = int(rng.choice([1, 2, 10, 100, 257, 1000, 1024]))
+    codes = rng.integers(0, 256, size=(N, M), dtype=np.uint8)
+    cb = rng.integers(0, 16, size=(M, 256, dsub)).astype(np.float32)
+    q = rng.integers(0, 16, size=(B, M * dsub)).astype(np.float32)
+    lists = []
+    budget = 1_500_000
+    for b in range(B):
+        kind = rng.integers(0, 6)
+        n = int(min(budget // B * 2, rng.choice([0, 1, 30, 700, 9_000, 40_000, 150_000])))
+        if kind == 0:
+            x = rng.integers(0, N, n)                                               # spread, natural repeats
+        elif kind == 1:
+            x = rng.integers(0, max(1, N // 50), n)                                 # bunched at the bottom: heavy repeats
+        elif kind == 2:
+            x = N - 1 - rng.integers(0, max(1, N // 7), n)                          # bunched at the top
+        elif kind == 3:
+            x = np.repeat(rng.integers(0, N, max(1, n // 5)), 5)[:n]                # every ID five times in a row
+        elif kind == 4:
+            x = np.sort(rng.integers(0, N, n))                                      # ascending
+        else:
+            x = np.concatenate([rng.integers(0, N, n // 2), rng.integers(N, 2 ** 32 - 1, n - n // 2)])   # half invalid
+        x = x.astype(np.uint32)
+        if n and kind != 5 and rng.random() < 0.5:
+            x[rng.integers(0, n, max(1, n // 100))] = NONE                          # padding entries
+        lists.append(x)
+    off = np.zeros(B + 1, dtype=np.int64)
+    off[1:] = np.cumsum([len(x) for x in lists])
+    ids = np.concatenate(lists) if off[-1] else np.zeros(0, np.uint32)
+    ix = fann.FannIndex(0)
+    ix.load_codes(torch.from_numpy(codes).to(DEV))
+    lut = ix.build_lut(torch.from_numpy(q).to(DEV), torch.from_numpy(cb).to(DEV))
+    assert np.array_equal(lut.cpu().numpy(), oracle.build_lut(q, cb).astype(np.float32)), "integer tables must be exact"
+    ids_dev = torch.from_numpy(ids.view(np.int32)).to(DEV) if ids.size else torch.zeros(1, dtype=torch.int32, device=DEV)
+    o = ix.dedup_scan_topk(lut, torch.from_numpy(off).to(DEV), ids_dev, k, total_cands=int(off[-1]), check=True)
+    torch.cuda.synchronize()
+    ref = oracle.search(q, cb, codes, off, ids, k)
+    check_exact((np_u32(o[0]), o[1].cpu().numpy(), np_u32(o[2]), np_u32(o[3])), ref)
+    ix.close()
+
+
 def test_argument_errors(fann, tiny):
     w = tiny
     ix = fann.FannIndex(0)
