@@ -371,7 +371,26 @@ def time_device_path(fann, cfg, args, rank, local_rank, world, dev, keep_lists=F
     from workloads import DEFAULT_SEED, make_workload
     t_gen = time.time()
     by_window = getattr(args, "query_order", "generated") == "window"
-    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev, keep_lists=keep_lists or by_window)   # each replica: its own batch
+    lists_sorted = getattr(args, "list_order", "generated") == "ascending"
+    w = make_workload(cfg, seed=rank_seed(DEFAULT_SEED, rank), device=dev,
+                      keep_lists=keep_lists or by_window or lists_sorted)   # each replica: its own batch
+    if lists_sorted:
+        # measurement variant: every posting list stored in ascending ID order (a list's order carries no meaning,
+        # PAPER.md:L150; fann_load_lists does the same to its own copy): 32 consecutive candidates then fall into
+        # few ID-range classes, which is what the class split's MATCH instruction pays for
+        from workloads.generate import PostingLists, make_candidates
+        n_lists = w.list_offsets.numel() - 1
+        step = max(1, n_lists // 16)                               # a sixteenth of the lists at a time: bounded scratch
+        for l0 in range(0, n_lists, step):
+            l1 = min(n_lists, l0 + step)
+            e0, e1 = int(w.list_offsets[l0]), int(w.list_offsets[l1])
+            lens = w.list_offsets[l0 + 1:l1 + 1] - w.list_offsets[l0:l1]
+            seg = torch.repeat_interleave(torch.arange(l1 - l0, device=dev), lens)
+            key = (seg << 32) | (w.list_ids[e0:e1].long() & 0xFFFFFFFF)
+            w.list_ids[e0:e1] = (torch.sort(key).values & 0xFFFFFFFF).to(torch.int32)
+            del key, seg, lens
+        w.cand_offsets, w.cand_ids = make_candidates(cfg, PostingLists(w.list_offsets, w.list_ids, 0), w.probes.long())
+        torch.cuda.empty_cache()                                   # the library allocates outside torch's pool
     if by_window:
         # measurement variant: the same queries, ordered by the position of their probed window, so that queries
         # which share posting lists -- and code rows -- are scanned at about the same time (L2 reuse)
@@ -676,6 +695,8 @@ def main():
                     help="measurement only: the row-gather ceiling sweep on a synthetic array of the workload's size")
     ap.add_argument("--query-order", default="generated", choices=["generated", "window"],
                     help="measurement variant: 'window' orders the batch's queries by the position of their probed lists")
+    ap.add_argument("--list-order", default="generated", choices=["generated", "ascending"],
+                    help="measurement variant: 'ascending' stores every posting list in ascending ID order")
     ap.add_argument("--id-map", default=None, choices=["feistel", "lattice"],
                     help="vector -> ID map of the generator (default: the config's, 'feistel')")
     args = ap.parse_args()
@@ -850,7 +871,7 @@ def main():
         "ms_per_step": round(ms_per_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "N": cfg.N, "d": cfg.d, "M": M, "B": B, "nprobe": cfg.nprobe, "k": k,
-                   "id_map": cfg.id_map, "query_order": args.query_order, "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
+                   "id_map": cfg.id_map, "query_order": args.query_order, "list_order": args.list_order, "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                    "l2": res["l2"], "C_total": total, "U_total": U_total,
                    "distinct_fraction": round(U_total / max(total, 1), 4),
                    "C_mean": stats["C_mean"], "C_max": stats["C_max"], "gen_seconds": res["gen_seconds"]},

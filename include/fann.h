@@ -124,7 +124,8 @@ size_t fann_workspace_bytes(const fann_index *ix, uint32_t B, uint64_t total_can
  *       then id ascending; the remaining slots hold (+inf, FANN_ID_NONE).
  * lut          device, [B][M][256] fp32 as written by fann_build_lut
  * cand_offsets device, [B+1] int64, non-decreasing, cand_offsets[0] == 0
- * cand_ids     device, [total_cands] uint32
+ * cand_ids     device, [total_cands] uint32 (any order; a caller that keeps each posting
+ *              list's IDs in ascending order gets a faster class split)
  * total_cands  host value == cand_offsets[B] (lets the call size its work
  *              without reading device memory)
  * out_ids      device, [B][k] uint32        out_dists  device, [B][k] fp32
